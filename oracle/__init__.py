@@ -1,0 +1,24 @@
+"""fp64 CPU oracle of the phase-tracking hot path (arxiv 1906.10598).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only ``tests/``, ``__graft_entry__.smoke()`` and the
+``cpu_baseline`` / ``--impl reference`` legs of ``bench.py`` may import this package.  It imports
+nothing from ``paper_1906_10598_b200`` and shares no code with the CUDA path.
+
+``oracle/pt_oracle.c`` holds the arithmetic (plain C, fp64, exact-integer Philox); this package
+only compiles it with gcc and marshals numpy arrays into it with ctypes.
+"""
+from .pt_oracle import (  # noqa: F401
+    build,
+    cr32,
+    de_draws,
+    default_t0,
+    doppler_products,
+    fit_blocks,
+    fitness,
+    indices_from_words,
+    init_uniforms,
+    model,
+    num_threads,
+    philox4x32_10,
+    rss,
+)
