@@ -1,0 +1,167 @@
+/*
+ * pt.h -- C ABI of libpt.so: B200-native (sm_100a) phase tracking by Differential Evolution,
+ *         the data-parallel hot path of arxiv 1906.10598 ("The GPU-based Phase Tracking method for
+ *         Planetary Radio Science applications").  Citations are PAPER.md line numbers.
+ *
+ * Parameterisation.  theta = (a0, a1, phi0, f, fdot[, fddot]), D = 5 or 6, and the signal model is
+ *     s(t) = (a0 + a1 t) cos(phi0 + 2 pi (f t + fdot t^2/2 + fddot t^3/6)),   t in [-T/2, T/2)
+ * which is PAPER.md:128-137 (Eq. 2-3) with c0 = phi0, c1 = 2 pi f, c2 = pi fdot, c3 = (pi/3) fddot,
+ * c4 = a0, c5 = a1.  Sample n of a block sits at t_n = t0 + n/fs; t0 = -N/(2 fs) puts sample N/2 at
+ * the block centre.
+ *
+ * Conventions (all entry points).
+ *   - Return value: PT_OK (0) or a negative pt_status.  Nothing throws, nothing aborts, nothing prints.
+ *     pt_last_error_string() describes the last failure of the calling thread.
+ *   - Unless a parameter is marked [host], every array pointer is a DEVICE pointer owned by the caller
+ *     (the Python binding allocates them with torch).  Layouts are dense row-major.  Inputs are never
+ *     modified.  The library keeps no device memory between calls; scratch is passed in by the caller and
+ *     sized by the *_workspace_bytes query.
+ *   - Device entry points are asynchronous on the given stream and never synchronise the device.
+ *     The *_host entry point is synchronous and owns its temporary device memory.
+ *   - The stream argument is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - There is no CPU fallback: without a CUDA device every compute call returns PT_ERR_CUDA.
+ */
+#ifndef PT_H_
+#define PT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define PT_API __attribute__((visibility("default")))
+#else
+#define PT_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    PT_OK = 0,
+    PT_ERR_INVALID_ARG = -1, /* null pointer, N odd or < 8, D not 5/6, NP < 4, lo > hi, fs <= 0, F or CR out of range */
+    PT_ERR_UNSUPPORTED = -2, /* NP or N beyond the compiled limits, workspace too small                               */
+    PT_ERR_CUDA = -3         /* a CUDA call failed; see pt_last_error_string()                                        */
+} pt_status;
+
+#define PT_MAX_NP 1024      /* population limit of the DE kernel                                  */
+#define PT_PER_BLOCK_COLS 10 /* columns of pt_doppler_products' per_block output                  */
+
+/* DE control record: the paper's Table 4 plus the population size it never states. */
+typedef struct {
+    int32_t D;           /* 5: (a0,a1,phi0,f,fdot)   6: (+fddot)                     PAPER.md:213 Dim_XC */
+    int32_t NP;          /* population size, 4 <= NP <= PT_MAX_NP                                         */
+    int32_t generations; /* itermax; the fixed-count stop rule  */
+    double F;            /* mutation scaling factor F_XC, in [0, 2]         */
+    double CR;           /* crossover factor CR_XC, in [0, 1]         */
+    uint64_t seed;       /* Philox4x32-10 key (low word, high word)                                       */
+    double t0;           /* time of sample 0 relative to the block centre [s]; -N/(2 fs) by default       */
+} pt_de_config;
+
+/*
+ * pt_fitness -- the chi^2 objective with sigma_i = 1 (Eq. 4):
+ *     fitness[b][i] = sum_n ( x[b][n] - s(pop[b][i], t_n) )^2 .
+ * x        [B][N]      fp32 baseband samples (PAPER.md:121 data block; N even, N >= 8)
+ * pop      [B][NP][D]  fp32 ABSOLUTE parameter values (no per-block offset), so that a reference
+ *                      implementation can be fed exactly the same numbers
+ * fitness  [B][NP]     fp32 out
+ * Runs the same per-sample code as the DE kernel: fp32 FMA + one hardware cosine per sample and candidate,
+ * phase taken relative to a per-block fp64 reference trajectory.  Blocks larger than shared memory are
+ * streamed; then workspace (>= pt_fitness_workspace_bytes) is required, else it may be NULL.
+ */
+PT_API size_t pt_fitness_workspace_bytes(int64_t B, int32_t N, int32_t NP, int32_t D);
+PT_API int32_t pt_fitness(const float* x, int64_t B, int32_t N, double fs, double t0, const float* pop, int32_t NP,
+                   int32_t D, float* fitness, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * pt_fit_blocks -- Differential Evolution fit of every block (PAPER.md:39-43 Fig. 1, :203-224 Table 4):
+ * DE/rand/1/bin, NP members drawn uniformly in the box [lo, hi], then `generations`
+ * synchronous generations of mutation v = x_r1 + F (x_r2 - x_r3), binomial crossover with factor CR,
+ * reflect-then-clamp bound handling, chi^2 evaluation (Eq. 4) and greedy selection (accept on <=).
+ * Random numbers are Philox4x32-10 with counter (slot, candidate, generation, block_index) and key = seed,
+ * so every draw is independent of any floating-point decision.
+ * x            [B][N]     fp32 samples
+ * lo, hi       [B][D]     fp64 parameter box per block (XCmin / XCmax); lo == hi is legal
+ * block_index  [B]        u32 Philox counter word of each block, or NULL for 0..B-1
+ * best         [B][D]     fp64 out: member with the smallest RSS (lowest index on ties)
+ * best_rss     [B]        fp32 out: its RSS (the "RSS" column of the paper's output record)
+ * status       [B]        u32 out: bit0 = best lies within 1e-6 (hi-lo) of a box face;
+ *                                  bit1 = population not collapsed (max RSS - min RSS > 1e-6 min RSS)
+ * final_pop    [B][NP][D] fp32 out, optional (NULL): final population rounded to fp32
+ * final_fit    [B][NP]    fp32 out, optional (NULL)
+ * workspace               >= pt_fit_blocks_workspace_bytes(B, N, cfg) bytes of device scratch (may be NULL if 0)
+ */
+PT_API size_t pt_fit_blocks_workspace_bytes(int64_t B, int32_t N, const pt_de_config* cfg /*[host]*/);
+PT_API int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const double* lo, const double* hi,
+                      const uint32_t* block_index, const pt_de_config* cfg /*[host]*/, double* best,
+                      float* best_rss, uint32_t* status, float* final_pop, float* final_fit, void* workspace,
+                      size_t workspace_bytes, void* stream);
+
+/*
+ * pt_doppler_products -- observables from the fitted parameters, fp64 throughout.  T = N/fs.
+ *     phi(t) = phi0 + 2 pi (f t + fdot t^2/2 + fddot t^3/6),  F(t) = dphi/dt  [rad/s]    PAPER.md:228-234 (Eq. 7)
+ *     border values at t = -T/2, +T/2, phases reduced to [0, 2 pi)                      PAPER.md:237-246 (Eq. 8)
+ *     dphi_block = phi(T/2) - phi(-T/2)                                                 PAPER.md:349 (Eq. 17 summand)
+ *     Phi_total = sum of m consecutive dphi_block,  F_int = Phi_total / (m T)           PAPER.md:343-351 (Eq. 16-17)
+ *     a_los = los_scale * fdot, los_scale = c/f0 (1-way) or c/(2 M2 f0) (3-way); 0 skips  PAPER.md:376-378 (Eq. 19)
+ * best         [B][D]   fp64 fitted parameters (as written by pt_fit_blocks)
+ * per_block    [B][10]  fp64 out: f, fdot, a_los, phi(-T/2) mod 2pi, phi(+T/2) mod 2pi, F(-T/2), F(+T/2),
+ *                        dphi_block, border_dphi (to block b+1, wrapped to (-pi, pi]), border_dF;
+ *                        the two border columns of the last block are NaN
+ * total_phase  [B]      fp64 out: inclusive running sum of dphi_block (total-count phase)
+ * blocks_per_interval [n_intervals] [host] int32: m_k = Tc_k / T
+ * interval_out [n_intervals] [host] array of DEVICE pointers; interval_out[k] is [floor(B/m_k)][2] fp64 out:
+ *                        (Phi_total, F_int) of each run of m_k blocks
+ */
+PT_API int32_t pt_doppler_products(const double* best, int64_t B, int32_t D, double T, double los_scale,
+                            const int32_t* blocks_per_interval /*[host]*/, int32_t n_intervals,
+                            double* per_block, double* total_phase, double* const* interval_out /*[host]*/,
+                            void* stream);
+
+/*
+ * pt_track_host -- the whole hot path on HOST buffers: copy x, lo, hi to the device, pt_fit_blocks,
+ * pt_doppler_products, copy the results back; synchronous.  Every pointer is a [host] pointer
+ * (pinned memory makes the copies asynchronous-capable, pageable memory works).  Outputs that are NULL are skipped.
+ * interval_out[k] is a [host] pointer to [floor(B/m_k)][2] fp64.
+ */
+PT_API int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, const double* lo, const double* hi,
+                      const pt_de_config* cfg, double los_scale, const int32_t* blocks_per_interval,
+                      int32_t n_intervals, double* best, float* best_rss, uint32_t* status, double* per_block,
+                      double* total_phase, double* const* interval_out);
+
+/*
+ * pt_de_draws -- debug/parity entry: the integer random draws the DE kernel uses, for Q queries.
+ * query  [Q][3]  u32 device: (block_index, generation >= 1, candidate)
+ * out    [Q][5]  i32 device: r1, r2, r3, jrand, crossover mask (bit j set = coordinate j takes the mutant)
+ * Runs the same device functions as pt_fit_blocks (Philox4x32-10, index map, CR threshold).
+ */
+PT_API int32_t pt_de_draws(const uint32_t* query, int64_t Q, int32_t NP, int32_t D, double CR, uint64_t seed,
+                    int32_t* out, void* stream);
+
+/*
+ * pt_init_population -- debug/parity entry: the generation-0 population of the DE kernel,
+ * pop0[B][NP][D] fp64 device = lo + (hi - lo) u, u = (Philox word >> 8) 2^-24.
+ */
+PT_API int32_t pt_init_population(const double* lo, const double* hi, const uint32_t* block_index, int64_t B, int32_t NP,
+                           int32_t D, uint64_t seed, double* pop0, void* stream);
+
+/*
+ * pt_peak_probe -- measured ALU peaks of the device, for the roofline denominators bench.py reports.
+ * kind 0: dependent-free FFMA stream; kind 1: MUFU.COS stream; kind 2: the 7 FP32 + 1 MUFU mix of one
+ * sample-evaluation.  Writes operations per second (fp32 lane-operations of the probed kind) to *ops_per_s [host].
+ * Synchronous.
+ */
+PT_API int32_t pt_peak_probe(int32_t kind, double* ops_per_s /*[host]*/);
+
+/* Launch geometry the library would use for pt_fit_blocks (for reporting): out[0] = grid, out[1] = threads per CTA,
+ * out[2] = dynamic shared memory bytes, out[3] = 1 if the block's samples stay resident in shared memory, 0 if streamed,
+ * out[4] = candidates per thread (register blocking), out[5] = CTAs per SM. */
+PT_API int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg /*[host]*/, int32_t out[6] /*[host]*/);
+
+PT_API const char* pt_last_error_string(void);
+PT_API const char* pt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PT_H_ */

@@ -1,0 +1,368 @@
+// pt_api.cu -- the C ABI of libpt.so (include/pt.h): argument checks, launch planning, kernel launches.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <cmath>
+#include <vector>
+
+#include "../../include/pt.h"
+#include "pt_de_kernel.cuh"
+#include "pt_internal.h"
+
+namespace pt {
+
+static thread_local char g_err[512] = "no error";
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+int check_cuda(cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return 0;
+    set_error("%s: %s", what, cudaGetErrorString(e));
+    return 1;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Launch plan of the block kernel.
+// ---------------------------------------------------------------------------------------------------
+struct Plan {
+    int C, threads, Wg, Ws, ctas_per_sm, grid, smem, Npad, NPpad, resident, sms;
+};
+
+static int device_info(int* sms, int* smem_optin) {
+    static int cached_dev = -1, c_sms = 0, c_smem = 0;
+    int dev = 0;
+    if (check_cuda(cudaGetDevice(&dev), "cudaGetDevice")) return 1;
+    if (dev != cached_dev) {
+        if (check_cuda(cudaDeviceGetAttribute(&c_sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute")) return 1;
+        if (check_cuda(cudaDeviceGetAttribute(&c_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev), "cudaDeviceGetAttribute")) return 1;
+        cached_dev = dev;
+    }
+    *sms = c_sms;
+    *smem_optin = c_smem;
+    return 0;
+}
+
+// Warp grid (Wg candidate-group columns x Ws sample slices) with the smallest per-warp load.
+static void choose_warp_grid(int warps, int groups, int nch, int* Wg, int* Ws) {
+    long long best = -1;
+    for (int wg = 1; wg <= warps; ++wg) {
+        if (warps % wg) continue;
+        const int ws = warps / wg;
+        const long long load = (long long)((groups + wg - 1) / wg) * ((nch + ws - 1) / ws);
+        // prefer fewer slices on ties (fewer partial sums to combine)
+        if (best < 0 || load < best || (load == best && ws < *Ws)) { best = load; *Wg = wg; *Ws = ws; }
+    }
+}
+
+// sms / smem_optin are passed in so that the plan can also be computed without a device (defaults of B200).
+static int make_plan(long long B, int N, int NP, int D, int sms, int smem_optin, Plan* pl) {
+    pl->sms = sms;
+    pl->C = (NP % 8 == 0) ? 8 : 4;
+    pl->NPpad = (NP + pl->C - 1) / pl->C * pl->C;
+    pl->Npad = (N + kChunk - 1) / kChunk * kChunk;
+    const int groups = pl->NPpad / pl->C, nch = pl->Npad / kChunk;
+    const int per_sm_total = smem_optin + 1024;   // 228 KB per SM, 1 KB reserved per resident CTA
+    int chosen = 0;
+    for (int cps = 4; cps >= 1; cps >>= 1) {
+        if (cps > 1 && B <= (long long)sms * (cps / 2)) continue;   // not enough blocks to want that many CTAs
+        const int threads = 512 / cps, warps = threads / 32;
+        int Wg = 1, Ws = warps;
+        choose_warp_grid(warps, groups, nch, &Wg, &Ws);
+        const SmemLayout L(pl->Npad, NP, pl->NPpad, D, Ws);
+        if (L.total > smem_optin) continue;
+        if ((long long)(L.total + 1024) * cps > per_sm_total) continue;
+        pl->threads = threads; pl->Wg = Wg; pl->Ws = Ws; pl->ctas_per_sm = cps; pl->smem = L.total;
+        chosen = 1;
+        break;
+    }
+    pl->resident = chosen;
+    if (!chosen) return 1;
+    const long long want = (long long)sms * pl->ctas_per_sm;
+    pl->grid = (int)(B < want ? B : want);
+    return 0;
+}
+
+template <int C, int D, int MODE>
+static int launch_block_kernel(const BlockParams& p, const Plan& pl, cudaStream_t st) {
+    static int configured_smem = -1;
+    if (pl.smem > configured_smem) {
+        if (check_cuda(cudaFuncSetAttribute(pt_block_kernel<C, D, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem),
+                       "cudaFuncSetAttribute"))
+            return PT_ERR_CUDA;
+        configured_smem = pl.smem;
+    }
+    pt_block_kernel<C, D, MODE><<<pl.grid, pl.threads, pl.smem, st>>>(p);
+    if (check_cuda(cudaGetLastError(), "pt_block_kernel launch")) return PT_ERR_CUDA;
+    return PT_OK;
+}
+
+template <int MODE>
+static int dispatch(const BlockParams& p, const Plan& pl, int D, cudaStream_t st) {
+    if (pl.C == 8) return D == 5 ? launch_block_kernel<8, 5, MODE>(p, pl, st) : launch_block_kernel<8, 6, MODE>(p, pl, st);
+    return D == 5 ? launch_block_kernel<4, 5, MODE>(p, pl, st) : launch_block_kernel<4, 6, MODE>(p, pl, st);
+}
+
+static uint32_t cr32_of(double CR) {
+    const double v = floor(CR * 4294967296.0);
+    if (v >= 4294967295.0) return 0xFFFFFFFFu;
+    if (v <= 0.0) return 0u;
+    return (uint32_t)v;
+}
+
+static int check_common(long long B, int N, double fs, int NP, int D) {
+    if (B < 1) { set_error("B must be >= 1"); return PT_ERR_INVALID_ARG; }
+    if (N < 8 || (N & 1)) { set_error("N must be even and >= 8 (got %d)", N); return PT_ERR_INVALID_ARG; }
+    if (!(fs > 0.0)) { set_error("fs must be > 0"); return PT_ERR_INVALID_ARG; }
+    if (D != 5 && D != 6) { set_error("D must be 5 or 6 (got %d)", D); return PT_ERR_INVALID_ARG; }
+    if (NP < 4) { set_error("NP must be >= 4 (got %d)", NP); return PT_ERR_INVALID_ARG; }
+    if (NP > PT_MAX_NP) { set_error("NP = %d exceeds PT_MAX_NP = %d", NP, PT_MAX_NP); return PT_ERR_UNSUPPORTED; }
+    return PT_OK;
+}
+
+static int check_cfg(const pt_de_config* cfg) {
+    if (!cfg) { set_error("cfg is null"); return PT_ERR_INVALID_ARG; }
+    if (cfg->generations < 0) { set_error("generations must be >= 0"); return PT_ERR_INVALID_ARG; }
+    if (!(cfg->F >= 0.0 && cfg->F <= 2.0)) { set_error("F must be in [0, 2]"); return PT_ERR_INVALID_ARG; }
+    if (!(cfg->CR >= 0.0 && cfg->CR <= 1.0)) { set_error("CR must be in [0, 1]"); return PT_ERR_INVALID_ARG; }
+    if (!std::isfinite(cfg->t0)) { set_error("t0 must be finite"); return PT_ERR_INVALID_ARG; }
+    return PT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// small parity / debug kernels: same device functions as the DE kernel
+// ---------------------------------------------------------------------------------------------------
+template <int D>
+__global__ void de_draws_kernel(const uint32_t* __restrict__ q, long long Q, uint32_t NP, uint32_t CR32, uint32_t k0,
+                                uint32_t k1, int32_t* __restrict__ out) {
+    const long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (k >= Q) return;
+    const Draws d = de_draws<D>(q[3 * k + 2], q[3 * k + 1], q[3 * k + 0], NP, CR32, k0, k1);
+    out[5 * k + 0] = d.r1; out[5 * k + 1] = d.r2; out[5 * k + 2] = d.r3; out[5 * k + 3] = d.jrand;
+    out[5 * k + 4] = (int32_t)d.mask;
+}
+
+template <int D>
+__global__ void init_population_kernel(const double* __restrict__ lo, const double* __restrict__ hi,
+                                       const uint32_t* __restrict__ block_index, long long B, int NP, uint32_t k0,
+                                       uint32_t k1, double* __restrict__ pop0) {
+    const long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (k >= B * NP) return;
+    const long long b = k / NP;
+    const int i = (int)(k % NP);
+    double l[D], h[D], th[D];
+#pragma unroll
+    for (int j = 0; j < D; ++j) { l[j] = lo[b * D + j]; h[j] = hi[b * D + j]; }
+    init_member<D>((uint32_t)i, block_index ? block_index[b] : (uint32_t)b, k0, k1, l, h, th);
+#pragma unroll
+    for (int j = 0; j < D; ++j) pop0[k * D + j] = th[j];
+}
+
+__global__ void check_box_kernel(const double* __restrict__ lo, const double* __restrict__ hi, long long n, int* bad) {
+    const long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    if (!(lo[k] <= hi[k])) atomicExch(bad, 1);
+}
+
+}  // namespace pt
+
+using namespace pt;
+
+extern "C" {
+
+const char* pt_last_error_string(void) { return g_err; }
+const char* pt_version(void) { return "pt 0.1 (sm_100a)"; }
+
+size_t pt_fitness_workspace_bytes(int64_t, int32_t, int32_t, int32_t) { return 0; }
+
+int32_t pt_fitness(const float* x, int64_t B, int32_t N, double fs, double t0, const float* pop, int32_t NP, int32_t D,
+                   float* fitness, void* workspace, size_t workspace_bytes, void* stream) {
+    (void)workspace; (void)workspace_bytes;
+    if (!x || !pop || !fitness) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    int rc = check_common(B, N, fs, NP, D);
+    if (rc) return rc;
+    if (!std::isfinite(t0)) { set_error("t0 must be finite"); return PT_ERR_INVALID_ARG; }
+    int sms, smem_optin;
+    if (device_info(&sms, &smem_optin)) return PT_ERR_CUDA;
+    Plan pl;
+    if (make_plan(B, N, NP, D, sms, smem_optin, &pl)) {
+        set_error("block of N = %d samples with NP = %d does not fit in shared memory (streamed path not built yet)", N, NP);
+        return PT_ERR_UNSUPPORTED;
+    }
+    BlockParams p;
+    memset(&p, 0, sizeof(p));
+    p.x = x; p.pop_in = pop; p.fitness_out = fitness;
+    p.B = B; p.N = N; p.Npad = pl.Npad; p.NP = NP; p.NPpad = pl.NPpad; p.G = 0;
+    p.fs = fs; p.t0 = t0; p.Wg = pl.Wg; p.Ws = pl.Ws;
+    p.use_bulk = ((N % 4) == 0 && (reinterpret_cast<uintptr_t>(x) % 16) == 0) ? 1 : 0;
+    return dispatch<kModeFitness>(p, pl, D, (cudaStream_t)stream);
+}
+
+size_t pt_fit_blocks_workspace_bytes(int64_t, int32_t, const pt_de_config*) { return 0; }
+
+int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg, int32_t out[6]) {
+    if (!cfg || !out) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    int rc = check_common(B, N, 1.0, cfg->NP, cfg->D);
+    if (rc) return rc;
+    int sms = 148, smem_optin = 232448;
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) == cudaSuccess && dev_count > 0) {
+        if (device_info(&sms, &smem_optin)) return PT_ERR_CUDA;
+    } else {
+        (void)cudaGetLastError();
+    }
+    Plan pl;
+    if (make_plan(B, N, cfg->NP, cfg->D, sms, smem_optin, &pl)) {
+        set_error("block does not fit in shared memory");
+        return PT_ERR_UNSUPPORTED;
+    }
+    out[0] = pl.grid; out[1] = pl.threads; out[2] = pl.smem; out[3] = pl.resident; out[4] = pl.C; out[5] = pl.ctas_per_sm;
+    return PT_OK;
+}
+
+int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const double* lo, const double* hi,
+                      const uint32_t* block_index, const pt_de_config* cfg, double* best, float* best_rss,
+                      uint32_t* status, float* final_pop, float* final_fit, void* workspace, size_t workspace_bytes,
+                      void* stream) {
+    (void)workspace; (void)workspace_bytes;
+    if (!x || !lo || !hi || !best || !best_rss || !status) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    int rc = check_cfg(cfg);
+    if (rc) return rc;
+    rc = check_common(B, N, fs, cfg->NP, cfg->D);
+    if (rc) return rc;
+    int sms, smem_optin;
+    if (device_info(&sms, &smem_optin)) return PT_ERR_CUDA;
+    Plan pl;
+    if (make_plan(B, N, cfg->NP, cfg->D, sms, smem_optin, &pl)) {
+        set_error("block of N = %d samples with NP = %d does not fit in shared memory (streamed path not built yet)", N, cfg->NP);
+        return PT_ERR_UNSUPPORTED;
+    }
+    BlockParams p;
+    memset(&p, 0, sizeof(p));
+    p.x = x; p.lo = lo; p.hi = hi; p.block_index = block_index;
+    p.best = best; p.best_rss = best_rss; p.status = status; p.final_pop = final_pop; p.final_fit = final_fit;
+    p.B = B; p.N = N; p.Npad = pl.Npad; p.NP = cfg->NP; p.NPpad = pl.NPpad; p.G = cfg->generations;
+    p.fs = fs; p.t0 = cfg->t0; p.F = cfg->F;
+    p.CR32 = cr32_of(cfg->CR);
+    p.key0 = (uint32_t)(cfg->seed & 0xFFFFFFFFull); p.key1 = (uint32_t)(cfg->seed >> 32);
+    p.Wg = pl.Wg; p.Ws = pl.Ws;
+    p.use_bulk = ((N % 4) == 0 && (reinterpret_cast<uintptr_t>(x) % 16) == 0) ? 1 : 0;
+    return dispatch<kModeFit>(p, pl, cfg->D, (cudaStream_t)stream);
+}
+
+int32_t pt_doppler_products(const double* best, int64_t B, int32_t D, double T, double los_scale,
+                            const int32_t* blocks_per_interval, int32_t n_intervals, double* per_block,
+                            double* total_phase, double* const* interval_out, void* stream) {
+    if (!best || !per_block || !total_phase) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    if (B < 1 || (D != 5 && D != 6) || !(T > 0.0) || n_intervals < 0) { set_error("invalid B, D, T or n_intervals"); return PT_ERR_INVALID_ARG; }
+    if (n_intervals > 0 && (!blocks_per_interval || !interval_out)) { set_error("null interval arguments"); return PT_ERR_INVALID_ARG; }
+    for (int k = 0; k < n_intervals; ++k) {
+        if (blocks_per_interval[k] < 1) { set_error("blocks_per_interval[%d] must be >= 1", k); return PT_ERR_INVALID_ARG; }
+        if (B / blocks_per_interval[k] > 0 && !interval_out[k]) { set_error("interval_out[%d] is null", k); return PT_ERR_INVALID_ARG; }
+    }
+    doppler_launch(best, B, D, T, los_scale, blocks_per_interval, n_intervals, per_block, total_phase, interval_out,
+                   (cudaStream_t)stream);
+    if (check_cuda(cudaGetLastError(), "doppler kernels launch")) return PT_ERR_CUDA;
+    return PT_OK;
+}
+
+int32_t pt_de_draws(const uint32_t* query, int64_t Q, int32_t NP, int32_t D, double CR, uint64_t seed, int32_t* out,
+                    void* stream) {
+    if (!query || !out) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    if (Q < 1 || NP < 4 || (D != 5 && D != 6) || !(CR >= 0.0 && CR <= 1.0)) { set_error("invalid Q, NP, D or CR"); return PT_ERR_INVALID_ARG; }
+    const int thr = 128;
+    const unsigned grid = (unsigned)((Q + thr - 1) / thr);
+    const uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
+    if (D == 5) de_draws_kernel<5><<<grid, thr, 0, (cudaStream_t)stream>>>(query, Q, (uint32_t)NP, cr32_of(CR), k0, k1, out);
+    else de_draws_kernel<6><<<grid, thr, 0, (cudaStream_t)stream>>>(query, Q, (uint32_t)NP, cr32_of(CR), k0, k1, out);
+    if (check_cuda(cudaGetLastError(), "de_draws_kernel launch")) return PT_ERR_CUDA;
+    return PT_OK;
+}
+
+int32_t pt_init_population(const double* lo, const double* hi, const uint32_t* block_index, int64_t B, int32_t NP,
+                           int32_t D, uint64_t seed, double* pop0, void* stream) {
+    if (!lo || !hi || !pop0) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    if (B < 1 || NP < 1 || (D != 5 && D != 6)) { set_error("invalid B, NP or D"); return PT_ERR_INVALID_ARG; }
+    const int thr = 128;
+    const unsigned grid = (unsigned)((B * NP + thr - 1) / thr);
+    const uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
+    if (D == 5) init_population_kernel<5><<<grid, thr, 0, (cudaStream_t)stream>>>(lo, hi, block_index, B, NP, k0, k1, pop0);
+    else init_population_kernel<6><<<grid, thr, 0, (cudaStream_t)stream>>>(lo, hi, block_index, B, NP, k0, k1, pop0);
+    if (check_cuda(cudaGetLastError(), "init_population_kernel launch")) return PT_ERR_CUDA;
+    return PT_OK;
+}
+
+int32_t pt_peak_probe(int32_t kind, double* ops_per_s) {
+    if (!ops_per_s || kind < 0 || kind > 3) { set_error("invalid probe arguments"); return PT_ERR_INVALID_ARG; }
+    return peak_probe(kind, ops_per_s);
+}
+
+int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, const double* lo, const double* hi,
+                      const pt_de_config* cfg, double los_scale, const int32_t* blocks_per_interval, int32_t n_intervals,
+                      double* best, float* best_rss, uint32_t* status, double* per_block, double* total_phase,
+                      double* const* interval_out) {
+    if (!x || !lo || !hi) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    int rc = check_cfg(cfg);
+    if (rc) return rc;
+    rc = check_common(B, N, fs, cfg->NP, cfg->D);
+    if (rc) return rc;
+    if (n_intervals < 0 || (n_intervals > 0 && (!blocks_per_interval || !interval_out))) { set_error("invalid interval arguments"); return PT_ERR_INVALID_ARG; }
+    for (long long k = 0; k < B * cfg->D; ++k)
+        if (!(lo[k] <= hi[k])) { set_error("lo > hi at element %lld", k); return PT_ERR_INVALID_ARG; }
+    const int D = cfg->D;
+    const size_t nx = (size_t)B * N * sizeof(float), nbox = (size_t)B * D * sizeof(double);
+    // one device arena for everything
+    size_t off = 0;
+    auto take = [&off](size_t bytes) { size_t o = off; off += (bytes + 255) / 256 * 256; return o; };
+    const size_t o_x = take(nx), o_lo = take(nbox), o_hi = take(nbox), o_best = take(nbox);
+    const size_t o_rss = take((size_t)B * 4), o_st = take((size_t)B * 4), o_pb = take((size_t)B * 10 * 8), o_tp = take((size_t)B * 8);
+    std::vector<size_t> o_iv(n_intervals);
+    std::vector<long long> cnt(n_intervals);
+    for (int k = 0; k < n_intervals; ++k) {
+        if (blocks_per_interval[k] < 1) { set_error("blocks_per_interval[%d] must be >= 1", k); return PT_ERR_INVALID_ARG; }
+        cnt[k] = B / blocks_per_interval[k];
+        o_iv[k] = take((size_t)(cnt[k] > 0 ? cnt[k] : 1) * 16);
+    }
+    unsigned char* arena = nullptr;
+    if (check_cuda(cudaMalloc(&arena, off), "cudaMalloc")) return PT_ERR_CUDA;
+    cudaStream_t st = nullptr;
+    if (check_cuda(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking), "cudaStreamCreate")) { cudaFree(arena); return PT_ERR_CUDA; }
+    int ret = PT_OK;
+    std::vector<double*> d_iv(n_intervals > 0 ? n_intervals : 1, nullptr);
+    for (int k = 0; k < n_intervals; ++k) d_iv[k] = reinterpret_cast<double*>(arena + o_iv[k]);
+    do {
+        if (check_cuda(cudaMemcpyAsync(arena + o_x, x, nx, cudaMemcpyHostToDevice, st), "H2D x")) { ret = PT_ERR_CUDA; break; }
+        if (check_cuda(cudaMemcpyAsync(arena + o_lo, lo, nbox, cudaMemcpyHostToDevice, st), "H2D lo")) { ret = PT_ERR_CUDA; break; }
+        if (check_cuda(cudaMemcpyAsync(arena + o_hi, hi, nbox, cudaMemcpyHostToDevice, st), "H2D hi")) { ret = PT_ERR_CUDA; break; }
+        ret = pt_fit_blocks(reinterpret_cast<float*>(arena + o_x), B, N, fs, reinterpret_cast<double*>(arena + o_lo),
+                            reinterpret_cast<double*>(arena + o_hi), nullptr, cfg, reinterpret_cast<double*>(arena + o_best),
+                            reinterpret_cast<float*>(arena + o_rss), reinterpret_cast<uint32_t*>(arena + o_st), nullptr,
+                            nullptr, nullptr, 0, st);
+        if (ret) break;
+        ret = pt_doppler_products(reinterpret_cast<double*>(arena + o_best), B, D, (double)N / fs, los_scale,
+                                  blocks_per_interval, n_intervals, reinterpret_cast<double*>(arena + o_pb),
+                                  reinterpret_cast<double*>(arena + o_tp), d_iv.data(), st);
+        if (ret) break;
+        cudaError_t e = cudaSuccess;
+        if (best) e = cudaMemcpyAsync(best, arena + o_best, nbox, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && best_rss) e = cudaMemcpyAsync(best_rss, arena + o_rss, (size_t)B * 4, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && status) e = cudaMemcpyAsync(status, arena + o_st, (size_t)B * 4, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && per_block) e = cudaMemcpyAsync(per_block, arena + o_pb, (size_t)B * 80, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && total_phase) e = cudaMemcpyAsync(total_phase, arena + o_tp, (size_t)B * 8, cudaMemcpyDeviceToHost, st);
+        for (int k = 0; k < n_intervals && e == cudaSuccess; ++k)
+            if (cnt[k] > 0 && interval_out[k])
+                e = cudaMemcpyAsync(interval_out[k], arena + o_iv[k], (size_t)cnt[k] * 16, cudaMemcpyDeviceToHost, st);
+        if (check_cuda(e, "D2H results")) { ret = PT_ERR_CUDA; break; }
+        if (check_cuda(cudaStreamSynchronize(st), "pt_track_host")) { ret = PT_ERR_CUDA; break; }
+    } while (0);
+    if (ret != PT_OK) cudaStreamSynchronize(st);
+    cudaStreamDestroy(st);
+    cudaFree(arena);
+    return ret;
+}
+
+}  // extern "C"

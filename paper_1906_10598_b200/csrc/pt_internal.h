@@ -1,0 +1,21 @@
+// pt_internal.h -- declarations shared by the translation units of libpt.so (not part of the public ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "pt_device.cuh"
+
+namespace pt {
+
+// pt_doppler.cu
+int doppler_launch(const double* best, long long B, int D, double T, double los_scale, const int32_t* m, int n_intervals,
+                   double* per_block, double* total_phase, double* const* interval_out, cudaStream_t st);
+
+// pt_probe.cu
+int peak_probe(int kind, double* ops_per_s);
+
+// pt_api.cu
+void set_error(const char* fmt, ...);
+int check_cuda(cudaError_t e, const char* what);
+
+}  // namespace pt

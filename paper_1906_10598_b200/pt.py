@@ -1,0 +1,212 @@
+"""Thin ctypes binding of ``libpt.so`` (C ABI in ``include/pt.h``): argument marshalling only.
+
+Every function takes torch CUDA tensors (device memory and streams are torch's), passes their data
+pointers and the current CUDA stream to the entry point of the same name, and raises ``PtError`` on a
+non-zero status.  There is no CPU fallback: if ``libpt.so`` is missing it is built with nvcc; if it cannot
+be built or loaded, or no CUDA device is present, the call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+_lib = None
+
+
+class PtError(RuntimeError):
+    pass
+
+
+class DEConfig(C.Structure):
+    """Mirror of ``pt_de_config`` (include/pt.h)."""
+
+    _fields_ = [
+        ("D", C.c_int32),
+        ("NP", C.c_int32),
+        ("generations", C.c_int32),
+        ("F", C.c_double),
+        ("CR", C.c_double),
+        ("seed", C.c_uint64),
+        ("t0", C.c_double),
+    ]
+
+
+def lib():
+    """Load (building first if needed) the CUDA library.  Raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if not os.path.exists(path):
+        path = _build.build()
+    L = C.CDLL(path)
+    p, i32, i64, f64, u64, sz = C.c_void_p, C.c_int32, C.c_int64, C.c_double, C.c_uint64, C.c_size_t
+    L.pt_last_error_string.restype = C.c_char_p
+    L.pt_version.restype = C.c_char_p
+    L.pt_fitness_workspace_bytes.argtypes = [i64, i32, i32, i32]
+    L.pt_fitness_workspace_bytes.restype = sz
+    L.pt_fitness.argtypes = [p, i64, i32, f64, f64, p, i32, i32, p, p, sz, p]
+    L.pt_fitness.restype = i32
+    L.pt_fit_blocks_workspace_bytes.argtypes = [i64, i32, C.POINTER(DEConfig)]
+    L.pt_fit_blocks_workspace_bytes.restype = sz
+    L.pt_fit_blocks.argtypes = [p, i64, i32, f64, p, p, p, C.POINTER(DEConfig), p, p, p, p, p, p, sz, p]
+    L.pt_fit_blocks.restype = i32
+    L.pt_fit_blocks_plan.argtypes = [i64, i32, C.POINTER(DEConfig), p]
+    L.pt_fit_blocks_plan.restype = i32
+    L.pt_doppler_products.argtypes = [p, i64, i32, f64, f64, p, i32, p, p, p, p]
+    L.pt_doppler_products.restype = i32
+    L.pt_track_host.argtypes = [p, i64, i32, f64, p, p, C.POINTER(DEConfig), f64, p, i32, p, p, p, p, p, p]
+    L.pt_track_host.restype = i32
+    L.pt_de_draws.argtypes = [p, i64, i32, i32, f64, u64, p, p]
+    L.pt_de_draws.restype = i32
+    L.pt_init_population.argtypes = [p, p, p, i64, i32, i32, u64, p, p]
+    L.pt_init_population.restype = i32
+    L.pt_peak_probe.argtypes = [i32, p]
+    L.pt_peak_probe.restype = i32
+    _lib = L
+    return L
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise PtError("%s failed (%d): %s" % (what, rc, lib().pt_last_error_string().decode()))
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _dev(t: torch.Tensor, dtype, name: str) -> int:
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise PtError("%s must be a contiguous CUDA tensor of dtype %s" % (name, dtype))
+    return t.data_ptr()
+
+
+def default_t0(N: int, fs: float) -> float:
+    return -float(N) / (2.0 * float(fs))
+
+
+def make_config(*, D: int, NP: int, generations: int, F: float = 0.5, CR: float = 0.9, seed: int = 0,
+                t0: float) -> DEConfig:
+    return DEConfig(int(D), int(NP), int(generations), float(F), float(CR), int(seed), float(t0))
+
+
+def pt_fitness(x: torch.Tensor, fs: float, pop: torch.Tensor, t0: float | None = None) -> torch.Tensor:
+    """fitness[B][NP] fp32 of pop[B][NP][D] fp32 on x[B][N] fp32 (Eq. 4)."""
+    B, N = x.shape
+    _, NP, D = pop.shape
+    if pop.shape[0] != B:
+        raise PtError("pop must be [B][NP][D]")
+    if t0 is None:
+        t0 = default_t0(N, fs)
+    out = torch.empty((B, NP), dtype=torch.float32, device=x.device)
+    rc = lib().pt_fitness(_dev(x, torch.float32, "x"), B, N, float(fs), float(t0), _dev(pop, torch.float32, "pop"), NP, D,
+                          out.data_ptr(), None, 0, _stream())
+    _check(rc, "pt_fitness")
+    return out
+
+
+def pt_fit_blocks(x: torch.Tensor, fs: float, lo: torch.Tensor, hi: torch.Tensor, cfg: DEConfig, *,
+                  block_index: torch.Tensor | None = None, want_pop: bool = False) -> dict:
+    """DE fit of every block; returns dict(best[B][D] f64, best_rss[B] f32, status[B] i32-view of u32
+    [, final_pop[B][NP][D] f32, final_fit[B][NP] f32])."""
+    B, N = x.shape
+    D, NP = cfg.D, cfg.NP
+    if tuple(lo.shape) != (B, D) or tuple(hi.shape) != (B, D):
+        raise PtError("lo and hi must be [B][D]")
+    dev = x.device
+    best = torch.empty((B, D), dtype=torch.float64, device=dev)
+    best_rss = torch.empty(B, dtype=torch.float32, device=dev)
+    status = torch.empty(B, dtype=torch.int32, device=dev)
+    fpop = torch.empty((B, NP, D), dtype=torch.float32, device=dev) if want_pop else None
+    ffit = torch.empty((B, NP), dtype=torch.float32, device=dev) if want_pop else None
+    ws_bytes = lib().pt_fit_blocks_workspace_bytes(B, N, C.byref(cfg))
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev) if ws_bytes else None
+    bidx = None if block_index is None else _dev(block_index, torch.int32, "block_index")
+    rc = lib().pt_fit_blocks(_dev(x, torch.float32, "x"), B, N, float(fs), _dev(lo, torch.float64, "lo"),
+                             _dev(hi, torch.float64, "hi"), bidx, C.byref(cfg), best.data_ptr(), best_rss.data_ptr(),
+                             status.data_ptr(), fpop.data_ptr() if want_pop else None,
+                             ffit.data_ptr() if want_pop else None, ws.data_ptr() if ws is not None else None, ws_bytes,
+                             _stream())
+    _check(rc, "pt_fit_blocks")
+    out = {"best": best, "best_rss": best_rss, "status": status}
+    if want_pop:
+        out["final_pop"] = fpop
+        out["final_fit"] = ffit
+    return out
+
+
+def pt_fit_blocks_plan(B: int, N: int, cfg: DEConfig) -> dict:
+    out = (C.c_int32 * 6)()
+    _check(lib().pt_fit_blocks_plan(B, N, C.byref(cfg), out), "pt_fit_blocks_plan")
+    return dict(grid=out[0], threads=out[1], smem=out[2], resident=out[3], cands_per_thread=out[4], ctas_per_sm=out[5])
+
+
+def pt_doppler_products(best: torch.Tensor, T: float, los_scale: float = 0.0, blocks_per_interval=()):
+    """(per_block[B][10], total_phase[B], [interval tensors [floor(B/m)][2]]), all fp64 on the device."""
+    B, D = best.shape
+    dev = best.device
+    m = [int(v) for v in blocks_per_interval]
+    per_block = torch.empty((B, 10), dtype=torch.float64, device=dev)
+    total = torch.empty(B, dtype=torch.float64, device=dev)
+    outs = [torch.empty((B // v, 2), dtype=torch.float64, device=dev) for v in m]
+    m_arr = (C.c_int32 * max(len(m), 1))(*m)
+    ptrs = (C.c_void_p * max(len(m), 1))(*[o.data_ptr() if o.numel() else None for o in outs])
+    rc = lib().pt_doppler_products(_dev(best, torch.float64, "best"), B, D, float(T), float(los_scale), m_arr, len(m),
+                                   per_block.data_ptr(), total.data_ptr(), ptrs, _stream())
+    _check(rc, "pt_doppler_products")
+    return per_block, total, outs
+
+
+def pt_track_host(x, fs: float, lo, hi, cfg: DEConfig, los_scale: float = 0.0, blocks_per_interval=()):
+    """Whole hot path on HOST tensors (CPU torch tensors, ideally pinned): H2D, fit, products, D2H."""
+    B, N = x.shape
+    D = cfg.D
+    for t, dt, nm in ((x, torch.float32, "x"), (lo, torch.float64, "lo"), (hi, torch.float64, "hi")):
+        if t.is_cuda or t.dtype != dt or not t.is_contiguous():
+            raise PtError("%s must be a contiguous host tensor of dtype %s" % (nm, dt))
+    m = [int(v) for v in blocks_per_interval]
+    best = torch.empty((B, D), dtype=torch.float64)
+    best_rss = torch.empty(B, dtype=torch.float32)
+    status = torch.empty(B, dtype=torch.int32)
+    per_block = torch.empty((B, 10), dtype=torch.float64)
+    total = torch.empty(B, dtype=torch.float64)
+    outs = [torch.empty((B // v, 2), dtype=torch.float64) for v in m]
+    m_arr = (C.c_int32 * max(len(m), 1))(*m)
+    ptrs = (C.c_void_p * max(len(m), 1))(*[o.data_ptr() if o.numel() else None for o in outs])
+    rc = lib().pt_track_host(x.data_ptr(), B, N, float(fs), lo.data_ptr(), hi.data_ptr(), C.byref(cfg), float(los_scale),
+                             m_arr, len(m), best.data_ptr(), best_rss.data_ptr(), status.data_ptr(), per_block.data_ptr(),
+                             total.data_ptr(), ptrs)
+    _check(rc, "pt_track_host")
+    return {"best": best, "best_rss": best_rss, "status": status, "per_block": per_block, "total_phase": total,
+            "intervals": outs}
+
+
+def pt_de_draws(query: torch.Tensor, NP: int, D: int, CR: float, seed: int) -> torch.Tensor:
+    """query[Q][3] int32 (block_index, generation, candidate) -> [Q][5] int32 (r1, r2, r3, jrand, mask)."""
+    Q = query.shape[0]
+    out = torch.empty((Q, 5), dtype=torch.int32, device=query.device)
+    rc = lib().pt_de_draws(_dev(query, torch.int32, "query"), Q, NP, D, float(CR), int(seed), out.data_ptr(), _stream())
+    _check(rc, "pt_de_draws")
+    return out
+
+
+def pt_init_population(lo: torch.Tensor, hi: torch.Tensor, NP: int, seed: int,
+                       block_index: torch.Tensor | None = None) -> torch.Tensor:
+    B, D = lo.shape
+    out = torch.empty((B, NP, D), dtype=torch.float64, device=lo.device)
+    bidx = None if block_index is None else _dev(block_index, torch.int32, "block_index")
+    rc = lib().pt_init_population(_dev(lo, torch.float64, "lo"), _dev(hi, torch.float64, "hi"), bidx, B, NP, D, int(seed),
+                                  out.data_ptr(), _stream())
+    _check(rc, "pt_init_population")
+    return out
+
+
+def pt_peak_probe(kind: int) -> float:
+    v = C.c_double(0.0)
+    _check(lib().pt_peak_probe(int(kind), C.byref(v)), "pt_peak_probe")
+    return float(v.value)
