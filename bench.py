@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the phase-tracking hot path (DE fit of every block + Doppler products).
+
+One "step" = one pass of the whole hot path over one synthetic track: pt_fit_blocks (the persistent
+DE kernel) followed by pt_doppler_products.  Default workload = BASELINE.json config 2, the one-hour
+track the target is quoted on (3600 blocks x 16000 samples, NP = 128, D = 5, 1000 generations).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config2|config1|config3s]
+
+Prints ONE JSON line (rank 0).  `value` = candidate-sample fitness evaluations per second (whole job, inputs
+resident in HBM); `e2e` = the same metric through pt_track_host with pinned HOST buffers (copies inside the
+timed region); `roofline` = the DE kernel against the XU (MUFU) issue roofline of the B200;
+`cpu_baseline` = the fp64 oracle on the host cores on a bounded sample.
+Under torchrun each rank fits its own track (weak scaling; no data-path collective).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "candidate-sample fitness evals/sec"
+UNIT = "sample-evals/s"
+SM_COUNT = 148
+XU_LANES_PER_SM = 16            # MUFU lanes per SM (4 per sub-partition): one cosine per sample-evaluation
+SM_MAX_MHZ = 1965.0
+XU_PEAK = SM_COUNT * XU_LANES_PER_SM * SM_MAX_MHZ * 1e6     # 4.65e12 sample-evaluations/s, DESIGN.md "Roofline"
+# dram__bytes_read.sum + dram__bytes_write.sum of one pt_block_kernel launch, from the ncu capture in profiles/
+TRAFFIC_BYTES_PER_LAUNCH = {"config2": None}
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return json.load(fh)
+    except Exception:
+        return {}
+
+
+def make_workload(name: str, case: int):
+    from paper_1906_10598_b200 import workloads as W
+    if name == "config2":
+        return W.config2(case=case)
+    if name == "config1":
+        return W.config1(case=case)
+    if name == "config3s":       # a 3600-block slice of config 3 around the occultation (D = 6)
+        return W.config3(blocks=range(16200, 19800), case=case)
+    if name == "tiny":           # for CPU-side plumbing tests
+        return W.config2(blocks=range(4), case=case, generations=3)
+    raise SystemExit("unknown workload %s" % name)
+
+
+def sample_evals(wl) -> float:
+    return float(wl.B) * wl.de["NP"] * (wl.de["generations"] + 1) * wl.N
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons while the timed region runs (B200_PROFILING.md recipe)."""
+
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu_index = gpu_index
+        self.proc = None
+        self.lines = []
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu_index), "--query-gpu=" + self.FIELDS,
+                                          "--format=csv,noheader,nounits", "-lms", "200"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            tok = [t.strip() for t in ln.split(",")]
+            if len(tok) < 9:
+                continue
+            try:
+                sm.append(float(tok[1])); smax.append(float(tok[2])); power.append(float(tok[3]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, tok[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        busy = [c for c, p in zip(sm, power) if p >= 0.5 * max(power)] or sm
+        return {"sm_mhz": float(np.median(busy)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
+                "power_w_max": float(max(power)), "samples": len(sm)}
+
+
+def cpu_baseline(wl, budget_blocks=None, generations=200) -> dict:
+    """The fp64 oracle, as it stands, on the host cores: DE on the first `cores` blocks of the workload for a
+    reduced generation count (the metric is a rate, every generation costs the same)."""
+    import oracle
+    cores = oracle.num_threads()
+    nb = min(wl.B, budget_blocks or cores)
+    G = min(generations, wl.de["generations"])
+    t0 = time.perf_counter()
+    oracle.fit_blocks(wl.x[:nb], wl.fs, wl.lo[:nb], wl.hi[:nb], NP=wl.de["NP"], generations=G, F=wl.de["F"],
+                      CR=wl.de["CR"], seed=1, block_index=wl.block_index[:nb])
+    dt = time.perf_counter() - t0
+    units = float(nb) * wl.de["NP"] * (G + 1) * wl.N
+    return {"value": units / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "DE fit of blocks 0..%d of %s for %d of %d generations (fp64 C oracle, OpenMP over blocks), %.1f s"
+                      % (nb - 1, wl.name, G, wl.de["generations"], dt)}
+
+
+def run_reference(args, rank: int, world: int):
+    """--impl reference: the oracle on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    import oracle
+    from paper_1906_10598_b200 import workloads as W
+    cores = oracle.num_threads()
+    nb = max(1, min(cores, 64))
+    if args.workload == "config1":
+        wl = W.config1(blocks=range(min(nb, 60)))
+    elif args.workload == "config3s":
+        wl = W.config3(blocks=range(16200, 16200 + nb))
+    elif args.workload == "tiny":
+        wl = W.config2(blocks=range(2), generations=3)
+    else:
+        wl = W.config2(blocks=range(nb))
+    G = min(wl.de["generations"], args.ref_generations)
+    units = float(wl.B) * wl.de["NP"] * (G + 1) * wl.N
+    times = []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        res = oracle.fit_blocks(wl.x, wl.fs, wl.lo, wl.hi, NP=wl.de["NP"], generations=G, F=wl.de["F"], CR=wl.de["CR"],
+                                seed=1, block_index=wl.block_index)
+        oracle.doppler_products(res["best"], wl.T, 0.0, [1])
+        dt = time.perf_counter() - t0
+        if it >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * float(np.mean(times))
+    value = units / (ms * 1e-3)
+    sample = ("each step = DE fit of %d blocks of %s for %d of %d generations (fp64 C oracle, OpenMP over blocks)"
+              % (wl.B, wl.name, G, wl.de["generations"]))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(args.workload, wl, full=False),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(name: str, wl, full=True) -> dict:
+    return {"workload": "BASELINE.json config 2 (one-hour track)" if name == "config2" else name,
+            "blocks": wl.B if full else "%d (sample)" % wl.B, "samples_per_block": wl.N, "fs_hz": wl.fs,
+            "NP": wl.de["NP"], "D": wl.de["D"], "generations": wl.de["generations"], "F": wl.de["F"], "CR": wl.de["CR"],
+            "box": "literal +-20% around the analytic profile", "l2": "inputs_exceed_l2" if wl.x.nbytes > 126e6 else
+            "inputs_fit_l2 (block samples are staged once into shared memory; HBM traffic is negligible)",
+            "parallelism": "one persistent CTA per data block; ranks fit independent tracks"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config2")
+    ap.add_argument("--ref-generations", type=int, default=100)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    from paper_1906_10598_b200 import pt
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    pt.lib()                                              # fail loudly if the CUDA library is missing
+    wl = make_workload(args.workload, case=rank)          # every rank fits its own track
+    cfg = pt.make_config(D=wl.de["D"], NP=wl.de["NP"], generations=wl.de["generations"], F=wl.de["F"], CR=wl.de["CR"],
+                         seed=1 + rank, t0=wl.t0)
+    plan = pt.pt_fit_blocks_plan(wl.B, wl.N, cfg)
+    m_int = [max(1, int(round(tc / wl.T))) for tc in (1.0, 10.0, 60.0)]
+    x_h = torch.from_numpy(wl.x).pin_memory()
+    lo_h = torch.from_numpy(wl.lo).pin_memory()
+    hi_h = torch.from_numpy(wl.hi).pin_memory()
+    x, lo, hi = x_h.to(dev), lo_h.to(dev), hi_h.to(dev)
+    torch.cuda.synchronize()
+    units = sample_evals(wl)
+
+    def step(ev=None):
+        if ev:
+            ev[0].record()
+        r = pt.pt_fit_blocks(x, wl.fs, lo, hi, cfg)
+        if ev:
+            ev[1].record()
+        prod = pt.pt_doppler_products(r["best"], wl.T, 0.0, m_int)
+        if ev:
+            ev[2].record()
+        return r, prod
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    t_start = torch.cuda.Event(enable_timing=True)
+    t_end = torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_start.record()
+    for k in range(args.steps):
+        r, prod = step(evs[k])
+    t_end.record()
+    barrier()
+    clocks = sampler.stop()
+    total_ms = t_start.elapsed_time(t_end)
+    fit_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    prod_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    if dist is not None:
+        tt = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+    ms_per_step = total_ms / args.steps
+    value = units * world / (ms_per_step * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (H2D + fit + products + D2H inside the timed region) ----
+    e2e = None
+    if not args.no_e2e:
+        pt.pt_track_host(x_h, wl.fs, lo_h, hi_h, cfg, 0.0, m_int)          # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        n_e2e = max(1, min(args.steps, 2))
+        for _ in range(n_e2e):
+            out = pt.pt_track_host(x_h, wl.fs, lo_h, hi_h, cfg, 0.0, m_int)
+        barrier()
+        e2e_s = (time.perf_counter() - t0) / n_e2e
+        if dist is not None:
+            tt = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            e2e_s = float(tt.item())
+        h2d = x_h.numel() * 4 + lo_h.numel() * 8 + hi_h.numel() * 8
+        d2h = sum(v.numel() * v.element_size() for k, v in out.items() if k != "intervals") + \
+            sum(v.numel() * 8 for v in out["intervals"])
+        e2e = {"value": units * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "ms_per_step": 1e3 * e2e_s, "real_time_factor": wl.B * wl.T / e2e_s}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    achieved = units / (fit_ms * 1e-3)
+    sm_mhz = clocks.get("sm_mhz") or SM_MAX_MHZ
+    roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": XU_PEAK / 1e12, "unit": "T sample-evals/s (1 MUFU cosine each)",
+                "frac": achieved / XU_PEAK, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.workload),
+                "kernel": "pt_block_kernel<C=%d,D=%d,fit>" % (plan["cands_per_thread"], wl.de["D"]),
+                "kernel_ms": fit_ms, "peak_source": "derived: 148 SMs x 16 MUFU lanes x 1965 MHz (DESIGN.md); "
+                "MEASURED_PEAKS.json holds no ALU peak",
+                "frac_at_sampled_clock": achieved / (SM_COUNT * XU_LANES_PER_SM * sm_mhz * 1e6),
+                "fp32_flops_achieved_tflops": achieved * (10 if wl.de["D"] == 5 else 12) / 1e12}
+    try:
+        roofline["measured_mufu_peak"] = pt.pt_peak_probe(1) / 1e12
+        roofline["measured_ffma_peak_tflops"] = 2 * pt.pt_peak_probe(0) / 1e12
+    except Exception as exc:  # diagnostics only
+        roofline["probe_error"] = str(exc)
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic", "config": workload_config(args.workload, wl),
+            "real_time_factor": wl.B * wl.T * world / (ms_per_step * 1e-3),
+            "fitness_evals_per_s": value / wl.N, "fit_ms": fit_ms, "doppler_products_ms": prod_ms, "plan": plan,
+            "roofline": roofline, "clocks": clocks, "gpu_launches": args.steps * (3 + len([m for m in m_int if wl.B // m > 0])),
+            "peaks_file": _peaks().get("when")}
+    if e2e is not None:
+        line["e2e"] = e2e
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(wl)
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

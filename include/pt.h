@@ -86,7 +86,7 @@ PT_API int32_t pt_fitness(const float* x, int64_t B, int32_t N, double fs, doubl
  * best         [B][D]     fp64 out: member with the smallest RSS (lowest index on ties)
  * best_rss     [B]        fp32 out: its RSS (the "RSS" column of the paper's output record)
  * status       [B]        u32 out: bit0 = best lies within 1e-6 (hi-lo) of a box face;
- *                                  bit1 = population not collapsed (max RSS - min RSS > 1e-6 min RSS)
+ *                                  bit1 = population not collapsed (max RSS - min RSS > 1e-3 min RSS)
  * final_pop    [B][NP][D] fp32 out, optional (NULL): final population rounded to fp32
  * final_fit    [B][NP]    fp32 out, optional (NULL)
  * workspace               >= pt_fit_blocks_workspace_bytes(B, N, cfg) bytes of device scratch (may be NULL if 0)

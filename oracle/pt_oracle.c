@@ -285,7 +285,7 @@ static void fit_one_block(const float* x, uint32_t b, int32_t N, double fs, cons
         double w = hi[j] - lo[j];
         if (w > 0.0 && (v - lo[j] <= 1e-6 * w || hi[j] - v <= 1e-6 * w)) st |= 1u;
     }
-    if (fmax - fmin > 1e-6 * fmin) st |= 2u;
+    if (fmax - fmin > 1e-3 * fmin) st |= 2u;   /* DESIGN.md reading R7: 1e-3, not SURVEY's 1e-6 */
     *best_rss = fmin;
     *status = st;
     if (final_pop) memcpy(final_pop, pop, sizeof(double) * (size_t)NP * D);

@@ -1,0 +1,98 @@
+"""The C-ABI library builds for sm_100a, loads without a GPU and exports every symbol include/pt.h declares.
+No compute call is made here (there is no GPU on the CPU test box); argument validation that happens before
+any CUDA call is checked through the real entry points."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib_path():
+    from paper_1906_10598_b200 import build
+    return build.build()
+
+
+def _declared_symbols():
+    with open(os.path.join(ROOT, "include", "pt.h")) as fh:
+        text = fh.read()
+    names = re.findall(r"PT_API\s+[\w\s\*]+?\b(pt_\w+)\s*\(", text)
+    assert len(names) >= 10
+    return sorted(set(names))
+
+
+def test_header_declares_the_north_star_entry_points():
+    names = _declared_symbols()
+    for must in ("pt_fitness", "pt_fit_blocks", "pt_doppler_products", "pt_last_error_string"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol(lib_path):
+    lib = C.CDLL(lib_path)
+    for name in _declared_symbols():
+        assert hasattr(lib, name), name
+
+
+def test_header_compiles_as_plain_c(tmp_path):
+    src = tmp_path / "t.c"
+    src.write_text('#include "pt.h"\nint main(void){ pt_de_config c; c.D = 5; return (int)sizeof(c) - (int)sizeof(c); }\n')
+    import subprocess
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), "-c", str(src), "-o",
+                    str(tmp_path / "t.o")], check=True)
+
+
+def test_config_struct_layout_matches_binding():
+    from paper_1906_10598_b200.pt import DEConfig
+    # int32 x3, pad, double x2, uint64, double = 48 bytes with natural alignment
+    assert C.sizeof(DEConfig) == 48
+    assert DEConfig.F.offset == 16 and DEConfig.seed.offset == 32 and DEConfig.t0.offset == 40
+
+
+def test_argument_validation_needs_no_gpu(lib_path):
+    from paper_1906_10598_b200 import pt
+    L = pt.lib()
+    cfg = pt.make_config(D=5, NP=60, generations=10, t0=-0.5)
+    dummy = C.c_void_p(256)
+    # null pointers
+    assert L.pt_fit_blocks(None, 1, 1000, 1000.0, dummy, dummy, None, C.byref(cfg), dummy, dummy, dummy, None, None,
+                           None, 0, None) == -1
+    assert b"null" in L.pt_last_error_string()
+    # N odd / too small, D, NP, F, CR
+    def call(N=1000, cfg=cfg, fs=1000.0):
+        return L.pt_fit_blocks(dummy, 1, N, fs, dummy, dummy, None, C.byref(cfg), dummy, dummy, dummy, None, None, None,
+                               0, None)
+    assert call(N=1001) == -1
+    assert call(N=6) == -1
+    assert call(fs=0.0) == -1
+    assert call(cfg=pt.make_config(D=4, NP=60, generations=1, t0=0.0)) == -1
+    assert call(cfg=pt.make_config(D=5, NP=3, generations=1, t0=0.0)) == -1
+    assert call(cfg=pt.make_config(D=5, NP=60, generations=-1, t0=0.0)) == -1
+    assert call(cfg=pt.make_config(D=5, NP=60, generations=1, F=2.5, t0=0.0)) == -1
+    assert call(cfg=pt.make_config(D=5, NP=60, generations=1, CR=1.5, t0=0.0)) == -1
+    assert call(cfg=pt.make_config(D=5, NP=4096, generations=1, t0=0.0)) == -2       # beyond PT_MAX_NP
+    assert L.pt_fitness(dummy, 1, 1000, 1000.0, -0.5, dummy, 60, 7, dummy, None, 0, None) == -1
+    assert L.pt_doppler_products(dummy, 0, 5, 1.0, 0.0, None, 0, dummy, dummy, None, None) == -1
+    assert L.pt_doppler_products(dummy, 4, 5, -1.0, 0.0, None, 0, dummy, dummy, None, None) == -1
+    assert L.pt_version().startswith(b"pt ")
+
+
+def test_plan_is_computable_without_gpu(lib_path):
+    from paper_1906_10598_b200 import pt
+    cfg = pt.make_config(D=5, NP=128, generations=1000, t0=-0.5)
+    plan = pt.pt_fit_blocks_plan(3600, 16000, cfg)
+    assert plan["resident"] == 1 and plan["grid"] >= 148 and plan["threads"] % 32 == 0
+    assert plan["smem"] <= 232448
+
+
+def test_product_path_has_no_oracle_import():
+    """The package must not import, read or run anything under oracle/ (the oracle is test infrastructure)."""
+    pkg = os.path.join(ROOT, "paper_1906_10598_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                with open(os.path.join(dirpath, f)) as fh:
+                    text = fh.read()
+                assert "import oracle" not in text and "from oracle" not in text and "pt_oracle" not in text, f

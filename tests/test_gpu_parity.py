@@ -1,0 +1,437 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the ctypes binding) against the fp64 CPU oracle,
+element by element on the same seeded inputs.  Bars (BASELINE.json north_star / SURVEY.md 8(c)-(d)):
+  * RNG streams and trial-vector indices: bit-exact;
+  * generation-0 population: bit-exact in fp64;
+  * fitness on identical populations: <= 1e-4 relative (fp32 + hardware cosine vs fp64);
+  * fitted parameters vs the oracle on the same noisy block: |dphi0| < 5 mrad (wrapped), |df| < 1e-3 Hz;
+  * both vs the generating truth: within 4 Cramer-Rao sigma;
+  * Doppler products: <= 1e-9 relative on identical parameters.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1906_10598_b200 import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+FIT_REL_TOL = 1e-4      # north_star: "GPU fitness values must match the oracle within 1e-4 relative"
+PHI0_TOL = 5e-3         # rad
+F_TOL = 1e-3            # Hz
+
+
+@pytest.fixture(scope="module")
+def pt():
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu-marked tests need a CUDA device; there is no CPU fallback")
+    from paper_1906_10598_b200 import pt as _pt
+    _pt.lib()
+    return _pt
+
+
+def _cuda(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _wrap(d):
+    return (np.asarray(d) + np.pi) % (2 * np.pi) - np.pi
+
+
+def _crlb(theta, N, fs, sigma, D):
+    """Cramer-Rao 1-sigma bounds of the model's parameters in white noise (Fisher matrix of Eq. 2)."""
+    t = -N / (2 * fs) + np.arange(N) / fs
+    th = list(theta) + [0.0] * (6 - len(theta))
+    ph = th[2] + 2 * np.pi * (th[3] * t + th[4] * t * t / 2 + th[5] * t**3 / 6)
+    A = th[0] + th[1] * t
+    c, s = np.cos(ph), np.sin(ph)
+    J = [c, t * c, -A * s, -A * s * 2 * np.pi * t, -A * s * np.pi * t * t]
+    if D == 6:
+        J.append(-A * s * np.pi * t**3 / 3)
+    J = np.array(J)
+    cov = np.linalg.inv(J @ J.T / sigma**2)
+    return np.sqrt(np.diag(cov))
+
+
+# ----------------------------------------------------------------------------------------------
+# bit-exact integer work
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("NP,D,CR", [(4, 5, 0.9), (5, 6, 0.5), (60, 5, 0.9), (100, 5, 0.85), (128, 6, 0.9),
+                                     (512, 5, 1.0), (1024, 6, 0.0)])
+def test_de_draws_bit_exact(pt, NP, D, CR):
+    rng = np.random.default_rng(NP * 10 + D)
+    Q = 3000
+    q = np.stack([rng.integers(0, 40000, Q), rng.integers(1, 2000, Q), rng.integers(0, NP, Q)], axis=1).astype(np.int32)
+    q[:NP, 2] = np.arange(NP)                   # every candidate index at least once
+    q[0, 0] = 2**31 - 1                         # large block index
+    seed = 0xC0FFEE1234567 + NP
+    got = pt.pt_de_draws(_cuda(q), NP, D, CR, seed).cpu().numpy()
+    for k in range(Q):
+        exp = oracle.de_draws(seed, int(q[k, 0]), int(q[k, 1]), int(q[k, 2]), NP, D, CR)
+        assert tuple(int(v) for v in got[k]) == exp, (k, q[k])
+
+
+@pytest.mark.parametrize("D", [5, 6])
+def test_initial_population_bit_exact(pt, D):
+    rng = np.random.default_rng(D)
+    B, NP = 7, 33
+    lo = rng.uniform(-5, 5, (B, D))
+    hi = lo + rng.uniform(0, 3, (B, D))
+    hi[2, 1] = lo[2, 1]                          # zero-width coordinate
+    bidx = np.array([0, 1, 5, 77, 3599, 35999, 2**31 - 1], dtype=np.int32)
+    seed = 987654321987
+    got = pt.pt_init_population(_cuda(lo), _cuda(hi), NP, seed, _cuda(bidx)).cpu().numpy()
+    for b in range(B):
+        for i in range(NP):
+            u = oracle.init_uniforms(seed, int(bidx[b]), i, D)
+            assert np.array_equal(got[b, i], lo[b] + (hi[b] - lo[b]) * u)
+
+
+# ----------------------------------------------------------------------------------------------
+# fitness on identical populations
+# ----------------------------------------------------------------------------------------------
+def _fitness_case(pt, wl, NP, seed=0, spread=1.0):
+    rng = np.random.default_rng(seed)
+    D = wl.D
+    mid, half = 0.5 * (wl.lo + wl.hi), 0.5 * (wl.hi - wl.lo) * spread
+    pop = (mid[:, None, :] + half[:, None, :] * rng.uniform(-1, 1, size=(wl.B, NP, D))).astype(np.float32)
+    ref = oracle.fitness(wl.x, wl.fs, pop)
+    got = pt.pt_fitness(_cuda(wl.x), wl.fs, _cuda(pop)).cpu().numpy().astype(np.float64)
+    rel = np.abs(got - ref) / ref
+    return rel.max()
+
+
+def test_fitness_config0(pt):
+    assert _fitness_case(pt, W.config0(cases=range(6)), NP=60) < FIT_REL_TOL            # C = 4 path, ragged tail chunk
+    assert _fitness_case(pt, W.config0(cases=range(3), box="paper"), NP=64) < FIT_REL_TOL
+
+
+def test_fitness_config1_2_3(pt):
+    assert _fitness_case(pt, W.config1(blocks=[0, 30, 59]), NP=100) < FIT_REL_TOL       # N = 10000: 78 chunks + 16 samples
+    assert _fitness_case(pt, W.config2(blocks=[0, 1799, 3599]), NP=128) < FIT_REL_TOL   # C = 8 path, N = 16000
+    assert _fitness_case(pt, W.config3(blocks=[0, 17900, 18000, 35999]), NP=128) < FIT_REL_TOL   # D = 6
+    assert _fitness_case(pt, W.config3(blocks=[17000, 18100], box="paper"), NP=36) < FIT_REL_TOL
+
+
+@pytest.mark.parametrize("N,NP", [(8, 4), (130, 7), (1030, 13), (4096, 32), (16384, 512), (2048, 1024)])
+def test_fitness_ragged_sizes(pt, N, NP):
+    """Smallest sizes, N not a multiple of the 128-sample chunk, NP not a multiple of the register blocking."""
+    fs = float(N)
+    wl = W.single_tone_blocks(range(5), N, fs, config=4, f_range=(0.05 * N, 0.2 * N))
+    assert _fitness_case(pt, wl, NP=NP, seed=N) < FIT_REL_TOL
+
+
+def test_fitness_near_converged_population_is_much_tighter(pt):
+    """With the population collapsed around the optimum the offsets from the fp64 reference are tiny and the
+    fp32 evaluation agrees with fp64 far better than the bar."""
+    wl = W.config2(blocks=[10, 2000])
+    assert _fitness_case(pt, wl, NP=128, spread=1e-4) < 2e-6
+
+
+def test_fitness_unaligned_rows_take_the_non_bulk_path(pt):
+    wl = W.single_tone_blocks(range(3), 1002, 1002.0, config=4, f_range=(50, 200))     # N % 4 == 2
+    assert _fitness_case(pt, wl, NP=16) < FIT_REL_TOL
+
+
+# ----------------------------------------------------------------------------------------------
+# DE trajectories
+# ----------------------------------------------------------------------------------------------
+def _gpu_fit(pt, wl, *, generations=None, seed=0, want_pop=False, F=None, CR=None, NP=None):
+    de = dict(wl.de)
+    cfg = pt.make_config(D=de["D"], NP=NP or de["NP"], generations=de["generations"] if generations is None else generations,
+                         F=de["F"] if F is None else F, CR=de["CR"] if CR is None else CR, seed=seed, t0=wl.t0)
+    r = pt.pt_fit_blocks(_cuda(wl.x), wl.fs, _cuda(wl.lo), _cuda(wl.hi), cfg,
+                         block_index=_cuda(wl.block_index.astype(np.int32)), want_pop=want_pop)
+    torch.cuda.synchronize()
+    return {k: v.cpu().numpy() for k, v in r.items()}
+
+
+def _oracle_fit(wl, *, generations=None, seed=0, want_pop=False, F=None, CR=None, NP=None):
+    de = wl.de
+    return oracle.fit_blocks(wl.x, wl.fs, wl.lo, wl.hi, NP=NP or de["NP"],
+                             generations=de["generations"] if generations is None else generations,
+                             F=de["F"] if F is None else F, CR=de["CR"] if CR is None else CR, seed=seed,
+                             block_index=wl.block_index, want_pop=want_pop)
+
+
+def test_generation_zero_population_and_fitness(pt):
+    wl = W.config0(cases=range(4))
+    g = _gpu_fit(pt, wl, generations=0, seed=5, want_pop=True)
+    o = _oracle_fit(wl, generations=0, seed=5, want_pop=True)
+    assert np.array_equal(g["final_pop"], o["final_pop"].astype(np.float32))
+    assert np.max(np.abs(g["final_fit"] - o["final_fit"]) / o["final_fit"]) < FIT_REL_TOL
+    assert np.max(np.abs(g["best_rss"] - o["best_rss"]) / o["best_rss"]) < FIT_REL_TOL
+    assert np.array_equal(g["best"], o["best"])            # fp64 best is the fp64 member itself
+
+
+@pytest.mark.parametrize("D", [5, 6])
+def test_first_generations_follow_the_oracle_trajectory(pt, D):
+    """Mutation, crossover and bound handling run in fp64 without contraction, so until a selection decision
+    falls inside the fp32 fitness error the GPU population IS the oracle population."""
+    wl = W.config0(cases=range(4)) if D == 5 else W.config3(blocks=[17990, 18010], NP=60, generations=5)
+    for G, F, CR in ((1, 0.5, 0.9), (4, 1.7, 0.6)):
+        g = _gpu_fit(pt, wl, generations=G, seed=21, want_pop=True, F=F, CR=CR, NP=60)
+        o = _oracle_fit(wl, generations=G, seed=21, want_pop=True, F=F, CR=CR, NP=60)
+        same = np.all(g["final_pop"] == o["final_pop"].astype(np.float32), axis=-1)
+        assert same.mean() > 0.98, same.mean()
+        assert np.all(g["final_pop"] >= wl.lo[:, None, :].astype(np.float32) - 1e-6)
+        assert np.all(g["final_pop"] <= wl.hi[:, None, :].astype(np.float32) + 1e-6)
+
+
+def _check_fit_vs_oracle_and_truth(wl, g, o, n_sigma=4.0, extra_f_bias=None):
+    D = wl.D
+    dphi = _wrap(g["best"][:, 2] - o["best"][:, 2])
+    df = g["best"][:, 3] - o["best"][:, 3]
+    assert np.max(np.abs(dphi)) < PHI0_TOL, np.max(np.abs(dphi))
+    assert np.max(np.abs(df)) < F_TOL, np.max(np.abs(df))
+    assert np.max(np.abs(g["best_rss"] - o["best_rss"]) / o["best_rss"]) < FIT_REL_TOL
+    assert np.max(np.abs(g["best"][:, 0] - o["best"][:, 0])) < 1e-3
+    for k in range(wl.B):
+        sig = wl.meta["sigma_per_block"][k] if "sigma_per_block" in wl.meta else wl.sigma
+        sd = _crlb(wl.truth[k], wl.N, wl.fs, sig, D)
+        for res in (g, o):
+            # well-determined combinations: phi0 and f where the box is wide enough for the
+            # optimum to be interior; a face-pinned optimum is judged against the oracle only
+            if res["status"][k] & 1:
+                continue
+            bias_f = 0.0 if extra_f_bias is None else extra_f_bias[k]
+            assert abs(_wrap(res["best"][k, 2] - wl.truth[k, 2])) < n_sigma * sd[2] + 1e-3
+            assert abs(res["best"][k, 3] - wl.truth[k, 3] - bias_f) < n_sigma * sd[3]
+
+
+def test_fit_config0_32_seeds(pt):
+    """BASELINE config 0: NP = 60, D = 5, F = 0.5, CR = 0.9, 500 generations, box +-20 % around truth."""
+    wl = W.config0(cases=range(32))
+    g = _gpu_fit(pt, wl, seed=3)
+    o = _oracle_fit(wl, seed=3)
+    _check_fit_vs_oracle_and_truth(wl, g, o)
+    # status bit0 (best on a box face) is decided by the same rule on both sides, but the fp32 objective cannot
+    # resolve the last 1e-6 (hi-lo) of the approach to a face: the GPU flag implies the
+    # oracle's, and where the oracle sits on a face the GPU's best is next to the same face
+    assert np.all((g["status"] & 1) <= (o["status"] & 1))
+    w = wl.hi - wl.lo
+    on_face = np.minimum(o["best"] - wl.lo, wl.hi - o["best"]) <= 1e-6 * w
+    near = np.minimum(g["best"] - wl.lo, wl.hi - g["best"]) <= 5e-3 * w
+    assert np.all(near[on_face])
+    assert np.all((g["status"] & 2) == 0) and np.all((o["status"] & 2) == 0)
+    # noiseless: both recover the generating truth
+    wn = W.config0(cases=range(4), noiseless=True)
+    gn = _gpu_fit(pt, wn, seed=3)
+    assert np.max(np.abs(_wrap(gn["best"][:, 2] - wn.truth[:, 2]))) < 1e-4
+    assert np.max(np.abs(gn["best"][:, 3] - wn.truth[:, 3])) < 1e-5
+    assert np.max(gn["best_rss"]) < 1e-6
+
+
+def test_fit_config0_paper_box_and_table4_settings(pt):
+    """Robustness cases: paper-style box (phi0 in [-pi, pi]) and Table 4's F = 0.5, CR = 0.85, 200 its."""
+    wl = W.config0(cases=range(8), box="paper")
+    g = _gpu_fit(pt, wl, seed=8)
+    o = _oracle_fit(wl, seed=8)
+    _check_fit_vs_oracle_and_truth(wl, g, o)
+    wl = W.config0(cases=range(8))
+    g = _gpu_fit(pt, wl, seed=9, generations=200, CR=0.85)
+    o = _oracle_fit(wl, seed=9, generations=200, CR=0.85)
+    _check_fit_vs_oracle_and_truth(wl, g, o)
+
+
+def test_fit_config1_blocks(pt):
+    """Config 1 (N = 10000, NP = 100, 1000 generations) on three blocks; D = 5 on a cubic-frequency signal is
+    biased by T^2 f''/40."""
+    wl = W.config1(blocks=[0, 30, 59])
+    g = _gpu_fit(pt, wl, seed=2)
+    o = _oracle_fit(wl, seed=2)
+    bias = wl.T**2 * wl.meta["fddot_true"] / 40.0
+    assert np.all((g["status"] & 2) == 0) and np.all((o["status"] & 2) == 0)
+    _check_fit_vs_oracle_and_truth(wl, g, o, extra_f_bias=bias)
+
+
+def test_fit_config1_sidelobe_case_is_detectable_and_a_retry_fixes_it(pt):
+    """DE is a heuristic and the two sides follow the same trajectory only until a selection decision falls inside
+    the fp32 fitness error.  Known case: block 59 of config 1 (a +-278 Hz box searched for a 1 Hz wide lobe) with
+    seed 1 -- the oracle ends in the main lobe, the GPU trajectory in a neighbouring local optimum.  Such a block
+    is detectable (chi^2 well above the noise power) and the paper's remedy is to search again
+    (PAPER.md:252); a second GPU run with another seed lands on the oracle's optimum."""
+    wl = W.config1(blocks=[59])
+    o = _oracle_fit(wl, seed=1)
+    g1 = _gpu_fit(pt, wl, seed=1)
+    z = lambda rss: (rss - (wl.N - 5) * wl.sigma**2) / (wl.sigma**2 * np.sqrt(2.0 * wl.N))
+    assert abs(z(o["best_rss"][0])) < 3.0
+    if abs(g1["best_rss"][0] - o["best_rss"][0]) / o["best_rss"][0] > FIT_REL_TOL:
+        assert z(g1["best_rss"][0]) > 3.0                       # the miss is visible in the objective itself
+    g2 = _gpu_fit(pt, wl, seed=2)
+    assert abs(g2["best_rss"][0] - o["best_rss"][0]) / o["best_rss"][0] < FIT_REL_TOL
+    assert abs(_wrap(g2["best"][0, 2] - o["best"][0, 2])) < PHI0_TOL
+    assert abs(g2["best"][0, 3] - o["best"][0, 3]) < F_TOL
+
+
+def test_fit_config2_blocks(pt):
+    wl = W.config2(blocks=[0, 1800])
+    g = _gpu_fit(pt, wl, seed=2)
+    o = _oracle_fit(wl, seed=2)
+    _check_fit_vs_oracle_and_truth(wl, g, o)
+
+
+def test_fit_config3_blocks(pt):
+    """D = 6, T = 0.1 s: fdot / fddot / a1 are not observable -- parity is required on
+    phi0, f, a0 and the block phase increment only."""
+    wl = W.config3(blocks=[100, 17950])
+    g = _gpu_fit(pt, wl, seed=4)
+    o = _oracle_fit(wl, seed=4)
+    dphi = _wrap(g["best"][:, 2] - o["best"][:, 2])
+    assert np.max(np.abs(dphi)) < PHI0_TOL
+    assert np.max(np.abs(g["best"][:, 3] - o["best"][:, 3])) < F_TOL
+    T = wl.T
+    inc_g = 2 * np.pi * (g["best"][:, 3] * T + g["best"][:, 5] * T**3 / 24)
+    inc_o = 2 * np.pi * (o["best"][:, 3] * T + o["best"][:, 5] * T**3 / 24)
+    assert np.max(np.abs(inc_g - inc_o)) < 2 * np.pi * F_TOL * T + 1e-6
+    assert np.max(np.abs(g["best_rss"] - o["best_rss"]) / o["best_rss"]) < FIT_REL_TOL
+
+
+def test_zero_width_box_and_tiny_population(pt):
+    wl = W.config0(cases=range(2))
+    lo, hi = wl.lo.copy(), wl.hi.copy()
+    lo[:, 1] = hi[:, 1] = wl.truth[:, 1]        # a1 fixed
+    lo[1] = hi[1] = wl.truth[1]                 # block 1: every coordinate fixed
+    wl.lo, wl.hi = lo, hi
+    g = _gpu_fit(pt, wl, seed=6, NP=4, generations=30, want_pop=True)
+    o = _oracle_fit(wl, seed=6, NP=4, generations=30, want_pop=True)
+    assert np.all(g["best"][:, 1] == wl.truth[:, 1])
+    assert np.array_equal(g["best"][1], wl.truth[1])
+    assert g["status"][1] == 0 and o["status"][1] == 0
+    assert np.all(g["final_pop"][1] == wl.truth[1].astype(np.float32))
+    assert abs(g["best_rss"][1] - o["best_rss"][1]) / o["best_rss"][1] < FIT_REL_TOL
+
+
+def test_status_face_bit(pt):
+    wl = W.config0(cases=[1])
+    wl.lo[0, 3] = wl.truth[0, 3] + 0.05
+    wl.hi[0, 3] = wl.truth[0, 3] + 0.5
+    g = _gpu_fit(pt, wl, seed=3, NP=40, generations=300)
+    assert g["status"][0] & 1
+    assert abs(g["best"][0, 3] - wl.lo[0, 3]) <= 1e-6 * 0.45
+    g2 = _gpu_fit(pt, W.config0(cases=[2]), seed=3, NP=32, generations=2)
+    assert g2["status"][0] & 2                   # not collapsed after two generations
+
+
+def test_block_index_selects_the_stream_and_persistent_loop_is_consistent(pt):
+    """More blocks than resident CTAs: every CTA loops over several blocks; results must equal a one-block run."""
+    wl = W.single_tone_blocks(range(700), 256, 256.0, config=4, f_range=(20, 60))
+    wl.de = dict(NP=16, D=5, generations=12, F=0.5, CR=0.9)
+    g = _gpu_fit(pt, wl, seed=77, want_pop=True)
+    for k in (0, 299, 699):
+        sub = W.single_tone_blocks([k], 256, 256.0, config=4, f_range=(20, 60))
+        sub.de = wl.de
+        sub.block_index = np.array([k], dtype=np.uint32)
+        gk = _gpu_fit(pt, sub, seed=77, want_pop=True)
+        assert np.array_equal(gk["final_pop"][0], g["final_pop"][k])
+        assert np.array_equal(gk["best"][0], g["best"][k])
+    o = oracle.fit_blocks(wl.x[:5], wl.fs, wl.lo[:5], wl.hi[:5], NP=16, generations=12, seed=77, want_pop=True)
+    same = np.all(g["final_pop"][:5] == o["final_pop"].astype(np.float32), axis=-1)
+    assert same.mean() > 0.9
+
+
+# ----------------------------------------------------------------------------------------------
+# Doppler products
+# ----------------------------------------------------------------------------------------------
+def _compare_products(pt, best, T, los, m):
+    pb_o, tot_o, iv_o = oracle.doppler_products(best, T, los, m)
+    pb, tot, iv = pt.pt_doppler_products(_cuda(best), T, los, m)
+    pb, tot = pb.cpu().numpy(), tot.cpu().numpy()
+    assert np.isnan(pb[-1, 8]) and np.isnan(pb[-1, 9])
+    # phases mod 2 pi and wrapped residuals carry the absolute rounding of a phase of magnitude |phi|
+    scale = np.maximum(np.abs(pb_o), 1.0)
+    scale[:, [3, 4, 8]] = np.maximum(np.abs(pb_o[:, [7]]), 1.0)
+    err = np.abs(pb - pb_o) / scale
+    assert np.nanmax(err) < 1e-9
+    assert np.max(np.abs(tot - tot_o) / np.maximum(np.abs(tot_o), 1.0)) < 1e-9
+    for a, b in zip(iv, iv_o):
+        a = a.cpu().numpy()
+        assert a.shape == b.shape
+        if b.size:
+            assert np.max(np.abs(a - b) / np.maximum(np.abs(b), 1.0)) < 1e-9
+
+
+@pytest.mark.parametrize("B,D,T", [(1, 5, 1.0), (60, 5, 1.0), (3600, 5, 1.0), (36000, 6, 0.1), (100003, 6, 0.5)])
+def test_doppler_products_vs_oracle(pt, B, D, T):
+    rng = np.random.default_rng(B)
+    best = np.stack([rng.uniform(0.5, 1.5, B), rng.uniform(-0.1, 0.1, B), rng.uniform(-np.pi, np.pi, B),
+                     rng.uniform(1000, 5200, B), rng.uniform(-5, 5, B)] + ([rng.uniform(-1, 1, B)] if D == 6 else []),
+                    axis=1)
+    m = [max(1, int(round(tc / T))) for tc in (1.0, 10.0, 60.0)]
+    _compare_products(pt, best, T, 0.031, m)
+
+
+def test_doppler_products_appendix_a(pt, golden_dir):
+    """The paper's worked example through the CUDA path."""
+    from test_oracle_doppler import _read_appendix, _theta_from_paper_units
+    blocks, borders, _ = _read_appendix(golden_dir)
+    best = np.array([_theta_from_paper_units(r) for r in blocks])
+    pb, tot, _ = pt.pt_doppler_products(_cuda(best), 2.0)
+    pb = pb.cpu().numpy()
+    assert np.all(np.abs(pb[:, 7] - blocks[:, 7]) <= 1.5e-3)
+    assert np.all(np.abs(pb[:-1, 6] - borders[:, 2]) <= 3e-3)
+    assert np.all(np.abs(pb[1:, 5] - borders[:, 4]) <= 3e-3)
+    assert np.all(np.abs(_wrap(pb[1:, 3] - borders[:, 3])) <= 2.5e-3)
+
+
+# ----------------------------------------------------------------------------------------------
+# host-buffer entry point and integrated phase
+# ----------------------------------------------------------------------------------------------
+def test_track_host_equals_device_path_and_integrated_phase_config1(pt):
+    """Config 1 at full size (60 x 10000, NP = 100, 1000 generations) through pt_track_host; the 60 s integrated
+    phase is compared with the analytic integral minus the D = 5 truncation term."""
+    wl = W.config1()
+    cfg = pt.make_config(D=5, NP=100, generations=1000, seed=1, t0=wl.t0)
+    h = pt.pt_track_host(torch.from_numpy(wl.x), wl.fs, torch.from_numpy(wl.lo), torch.from_numpy(wl.hi), cfg, 0.0,
+                         [1, 10, 60])
+    g = _gpu_fit(pt, wl, seed=1)
+    assert np.array_equal(h["best"].numpy(), g["best"])
+    pb, tot, iv = pt.pt_doppler_products(_cuda(g["best"]), wl.T, 0.0, [1, 10, 60])
+    assert np.array_equal(h["total_phase"].numpy(), tot.cpu().numpy())
+    assert np.array_equal(h["intervals"][2].numpy(), iv[2].cpu().numpy())
+    phi60 = h["intervals"][2].numpy()[0, 0]
+    analytic = wl.meta["dphi_true"].sum()
+    trunc = np.sum(2 * np.pi * wl.meta["fddot_true"] * wl.T**3 / 60.0)
+    assert abs(phi60 - (analytic - trunc)) < 0.34          # 4 sqrt(60) sigma(dphi_block), SURVEY q16
+    assert abs(phi60 - iv[1].cpu().numpy()[:, 0].sum()) < 1e-6
+    # oracle products on the GPU's parameters
+    pb_o, tot_o, _ = oracle.doppler_products(g["best"], wl.T, 0.0, [1, 10, 60])
+    assert abs(tot_o[-1] - phi60) < 1e-6
+    # three of the blocks against the oracle's own fit
+    sub = W.config1(blocks=[7, 41])
+    o = _oracle_fit(sub, seed=1)
+    assert np.max(np.abs(_wrap(g["best"][[7, 41], 2] - o["best"][:, 2]))) < PHI0_TOL
+    assert np.max(np.abs(g["best"][[7, 41], 3] - o["best"][:, 3])) < F_TOL
+
+
+def test_full_size_config2_sampled_blocks(pt):
+    """BASELINE config 2 at full size in bench.py's launch configuration (3600 x 16000, NP = 128, 1000 generations):
+    sampled blocks are checked one by one with the oracle's objective; properties are checked on all blocks."""
+    wl = W.config2()
+    g = _gpu_fit(pt, wl, seed=1)
+    assert np.all(np.isfinite(g["best"])) and np.all(np.isfinite(g["best_rss"]))
+    assert np.all(g["best"] >= wl.lo) and np.all(g["best"] <= wl.hi)
+    assert np.all((g["status"] & 2) == 0)                              # every population collapsed (1e-3 rule)
+    # chi^2 at the optimum is the summed noise power: (N - D) sigma^2 within 5 sigma, all blocks
+    z = (g["best_rss"] - (wl.N - 5) * wl.sigma**2) / (wl.sigma**2 * np.sqrt(2.0 * wl.N))
+    assert np.max(np.abs(z)) < 5.0 and abs(z.mean()) < 0.2
+    for k in range(0, 3600, 240):
+        r_or = oracle.rss(wl.x[k], wl.fs, g["best"][k])               # oracle's objective at the GPU's optimum
+        assert abs(g["best_rss"][k] - r_or) / r_or < FIT_REL_TOL
+        assert r_or <= oracle.rss(wl.x[k], wl.fs, wl.truth[k])        # at least as good as the generating truth
+    # border continuity (Eq. 8) at the noise level: phase residual sigma ~ 2 x 12 mrad x a few
+    pb, tot, iv = pt.pt_doppler_products(_cuda(g["best"]), wl.T, 0.0, [1, 10, 60])
+    pb = pb.cpu().numpy()
+    assert np.nanstd(pb[:, 8]) < 0.1
+    # 60-s integration Doppler against the analytic phase advance (truncation <= 1.3e-3 rad per 60 s)
+    phi60 = iv[2].cpu().numpy()[:, 0]
+    true60 = wl.meta["dphi_true"].reshape(60, 60).sum(axis=1)
+    sd_f = _crlb(wl.truth[1800], wl.N, wl.fs, wl.sigma, 5)[3]
+    sd60 = np.sqrt(60.0) * 2 * np.pi * sd_f * wl.T            # Eq. 17: sum of 60 independent block increments
+    assert np.max(np.abs(phi60 - true60)) < 4.5 * sd60
+    assert np.std(phi60 - true60) < 1.5 * sd60
+    # one sampled block against the oracle's own DE fit
+    sub = W.config2(blocks=[1234])
+    o = _oracle_fit(sub, seed=1)
+    assert abs(_wrap(g["best"][1234, 2] - o["best"][0, 2])) < PHI0_TOL
+    assert abs(g["best"][1234, 3] - o["best"][0, 3]) < F_TOL
