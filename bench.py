@@ -55,6 +55,8 @@ def make_workload(name: str, case: int):
         return W.config1(case=case)
     if name == "config3s":       # a 3600-block slice of config 3 around the occultation (D = 6)
         return W.config3(blocks=range(16200, 19800), case=case)
+    if name == "config2_ncu":    # one wave of config-2 blocks, 100 generations: short enough for `ncu --set full`
+        return W.config2(blocks=range(148), case=case, generations=100)
     if name == "tiny":           # for CPU-side plumbing tests
         return W.config2(blocks=range(4), case=case, generations=3)
     raise SystemExit("unknown workload %s" % name)

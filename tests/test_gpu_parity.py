@@ -245,23 +245,33 @@ def test_fit_config1_blocks(pt):
     _check_fit_vs_oracle_and_truth(wl, g, o, extra_f_bias=bias)
 
 
-def test_fit_config1_sidelobe_case_is_detectable_and_a_retry_fixes_it(pt):
+def test_fit_config1_block59_premature_convergence_is_a_valid_result_on_both_sides(pt):
     """DE is a heuristic and the two sides follow the same trajectory only until a selection decision falls inside
-    the fp32 fitness error.  Known case: block 59 of config 1 (a +-278 Hz box searched for a 1 Hz wide lobe) with
-    seed 1 -- the oracle ends in the main lobe, the GPU trajectory in a neighbouring local optimum.  Such a block
-    is detectable (chi^2 well above the noise power) and the paper's remedy is to search again
-    (PAPER.md:252); a second GPU run with another seed lands on the oracle's optimum."""
+    the fp32 fitness error.  Known hard case: block 59 of config 1 (a +-278 Hz box searched for a 1 Hz wide lobe).
+    With seed 1 the ORACLE's population collapses early (a0 = 0.960, chi^2 = 512.49) while seeds 2-4 reach the
+    optimum (a0 = 1.004, chi^2 = 502.60); the paper's remedy for a doubtful block is to search again.
+    Several results are correct here, so: every run must be a VALID result (its chi^2 is the oracle's objective at
+    its own parameters, inside the box), both sides must reach the lowest optimum for at least one seed, and all
+    runs that reach it must agree at the parity bounds."""
     wl = W.config1(blocks=[59])
-    o = _oracle_fit(wl, seed=1)
-    g1 = _gpu_fit(pt, wl, seed=1)
-    z = lambda rss: (rss - (wl.N - 5) * wl.sigma**2) / (wl.sigma**2 * np.sqrt(2.0 * wl.N))
-    assert abs(z(o["best_rss"][0])) < 3.0
-    if abs(g1["best_rss"][0] - o["best_rss"][0]) / o["best_rss"][0] > FIT_REL_TOL:
-        assert z(g1["best_rss"][0]) > 3.0                       # the miss is visible in the objective itself
-    g2 = _gpu_fit(pt, wl, seed=2)
-    assert abs(g2["best_rss"][0] - o["best_rss"][0]) / o["best_rss"][0] < FIT_REL_TOL
-    assert abs(_wrap(g2["best"][0, 2] - o["best"][0, 2])) < PHI0_TOL
-    assert abs(g2["best"][0, 3] - o["best"][0, 3]) < F_TOL
+    runs = {}
+    for seed in (1, 2, 3):
+        runs[("oracle", seed)] = _oracle_fit(wl, seed=seed)
+        runs[("gpu", seed)] = _gpu_fit(pt, wl, seed=seed)
+    rss = {}
+    for k, v in runs.items():
+        rss[k] = float(v["best_rss"][0])
+        r = oracle.rss(wl.x[0], wl.fs, v["best"][0])
+        assert abs(rss[k] - r) / r < FIT_REL_TOL, k
+        assert np.all(v["best"][0] >= wl.lo[0]) and np.all(v["best"][0] <= wl.hi[0]), k
+    lowest = min(rss.values())
+    at_optimum = [k for k in runs if rss[k] - lowest < FIT_REL_TOL * lowest]
+    assert any(k[0] == "oracle" for k in at_optimum) and any(k[0] == "gpu" for k in at_optimum), rss
+    ref = runs[[k for k in at_optimum if k[0] == "oracle"][0]]["best"][0]
+    for k in at_optimum:
+        assert abs(_wrap(runs[k]["best"][0, 2] - ref[2])) < PHI0_TOL, (k, rss)
+        assert abs(runs[k]["best"][0, 3] - ref[3]) < F_TOL, (k, rss)
+        assert abs(runs[k]["best"][0, 0] - ref[0]) < 1e-3, (k, rss)
 
 
 def test_fit_config2_blocks(pt):
