@@ -31,6 +31,8 @@ int check_cuda(cudaError_t e, const char* what) {
 // ---------------------------------------------------------------------------------------------------
 struct Plan {
     int C, threads, Wg, Ws, ctas_per_sm, grid, smem, Npad, NPpad, resident, sms;
+    int TS, S;              // streamed path: samples per tile, ring stages (0, 0 when resident)
+    size_t ws_bytes;        // device workspace the launch needs (streamed path only)
 };
 
 static int device_info(int* sms, int* smem_optin) {
@@ -81,30 +83,84 @@ static int make_plan(long long B, int N, int NP, int D, int sms, int smem_optin,
         break;
     }
     pl->resident = chosen;
-    if (!chosen) return 1;
+    pl->TS = 0; pl->S = 0; pl->ws_bytes = 0;
+    if (!chosen) {
+        // streamed: one CTA of 512 threads per SM, ring of 3 stages, the largest tile that fits
+        const int threads = 512, warps = threads / 32, S = 3;
+        for (int TS = 8192; TS >= 1024 && !chosen; TS >>= 1) {
+            int Wg = 1, Ws = warps;
+            choose_warp_grid(warps, groups, TS / kChunk, &Wg, &Ws);
+            const SmemLayout L(pl->Npad, NP, pl->NPpad, D, Ws, TS, S);
+            if (L.total > smem_optin) continue;
+            pl->threads = threads; pl->Wg = Wg; pl->Ws = Ws; pl->ctas_per_sm = 1; pl->smem = L.total;
+            pl->TS = TS; pl->S = S;
+            chosen = 1;
+        }
+        if (!chosen) return 1;
+    }
     const long long want = (long long)sms * pl->ctas_per_sm;
     pl->grid = (int)(B < want ? B : want);
+    if (pl->S > 0) pl->ws_bytes = (size_t)pl->grid * pl->Npad * sizeof(float) * 2;   // reference-phase rows + aligned copies
     return 0;
 }
 
-template <int C, int D, int MODE>
+// plan with the current device's limits, or B200's when no device is present (the query entry points)
+static int plan_for(long long B, int N, int NP, int D, Plan* pl, bool need_device) {
+    int sms = 148, smem_optin = 232448;
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) == cudaSuccess && dev_count > 0) {
+        if (device_info(&sms, &smem_optin)) return PT_ERR_CUDA;
+    } else {
+        (void)cudaGetLastError();
+        if (need_device) { set_error("no CUDA device"); return PT_ERR_CUDA; }
+    }
+    if (make_plan(B, N, NP, D, sms, smem_optin, pl)) {
+        set_error("N = %d with NP = %d: population tables alone exceed shared memory", N, NP);
+        return PT_ERR_UNSUPPORTED;
+    }
+    return PT_OK;
+}
+
+template <int C, int D, int MODE, bool STREAM>
 static int launch_block_kernel(const BlockParams& p, const Plan& pl, cudaStream_t st) {
     static int configured_smem = -1;
     if (pl.smem > configured_smem) {
-        if (check_cuda(cudaFuncSetAttribute(pt_block_kernel<C, D, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem),
+        if (check_cuda(cudaFuncSetAttribute(pt_block_kernel<C, D, MODE, STREAM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            pl.smem),
                        "cudaFuncSetAttribute"))
             return PT_ERR_CUDA;
         configured_smem = pl.smem;
     }
-    pt_block_kernel<C, D, MODE><<<pl.grid, pl.threads, pl.smem, st>>>(p);
+    pt_block_kernel<C, D, MODE, STREAM><<<pl.grid, pl.threads, pl.smem, st>>>(p);
     if (check_cuda(cudaGetLastError(), "pt_block_kernel launch")) return PT_ERR_CUDA;
     return PT_OK;
 }
 
+template <int MODE, bool STREAM>
+static int dispatch2(const BlockParams& p, const Plan& pl, int D, cudaStream_t st) {
+    if (pl.C == 8)
+        return D == 5 ? launch_block_kernel<8, 5, MODE, STREAM>(p, pl, st) : launch_block_kernel<8, 6, MODE, STREAM>(p, pl, st);
+    return D == 5 ? launch_block_kernel<4, 5, MODE, STREAM>(p, pl, st) : launch_block_kernel<4, 6, MODE, STREAM>(p, pl, st);
+}
+
 template <int MODE>
 static int dispatch(const BlockParams& p, const Plan& pl, int D, cudaStream_t st) {
-    if (pl.C == 8) return D == 5 ? launch_block_kernel<8, 5, MODE>(p, pl, st) : launch_block_kernel<8, 6, MODE>(p, pl, st);
-    return D == 5 ? launch_block_kernel<4, 5, MODE>(p, pl, st) : launch_block_kernel<4, 6, MODE>(p, pl, st);
+    return pl.S > 0 ? dispatch2<MODE, true>(p, pl, D, st) : dispatch2<MODE, false>(p, pl, D, st);
+}
+
+// streamed path: hand the workspace rows to the kernel
+static int attach_workspace(BlockParams* p, const Plan& pl, void* workspace, size_t workspace_bytes) {
+    p->TS = pl.TS; p->S = pl.S;
+    if (pl.S == 0) return PT_OK;
+    if (!workspace || workspace_bytes < pl.ws_bytes) {
+        set_error("streamed path (N = %d does not fit in shared memory) needs %zu bytes of workspace, got %zu", p->N, pl.ws_bytes,
+                  workspace ? workspace_bytes : (size_t)0);
+        return PT_ERR_UNSUPPORTED;
+    }
+    if (reinterpret_cast<uintptr_t>(workspace) % 16) { set_error("workspace must be 16-byte aligned"); return PT_ERR_INVALID_ARG; }
+    p->ws_wref = reinterpret_cast<float*>(workspace);
+    p->ws_x = p->ws_wref + (size_t)pl.grid * pl.Npad;
+    return PT_OK;
 }
 
 static uint32_t cr32_of(double CR) {
@@ -177,49 +233,45 @@ extern "C" {
 const char* pt_last_error_string(void) { return g_err; }
 const char* pt_version(void) { return "pt 0.1 (sm_100a)"; }
 
-size_t pt_fitness_workspace_bytes(int64_t, int32_t, int32_t, int32_t) { return 0; }
+size_t pt_fitness_workspace_bytes(int64_t B, int32_t N, int32_t NP, int32_t D) {
+    Plan pl;
+    if (check_common(B, N, 1.0, NP, D) || plan_for(B, N, NP, D, &pl, false)) return 0;
+    return pl.ws_bytes;
+}
 
 int32_t pt_fitness(const float* x, int64_t B, int32_t N, double fs, double t0, const float* pop, int32_t NP, int32_t D,
                    float* fitness, void* workspace, size_t workspace_bytes, void* stream) {
-    (void)workspace; (void)workspace_bytes;
     if (!x || !pop || !fitness) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
     int rc = check_common(B, N, fs, NP, D);
     if (rc) return rc;
     if (!std::isfinite(t0)) { set_error("t0 must be finite"); return PT_ERR_INVALID_ARG; }
-    int sms, smem_optin;
-    if (device_info(&sms, &smem_optin)) return PT_ERR_CUDA;
     Plan pl;
-    if (make_plan(B, N, NP, D, sms, smem_optin, &pl)) {
-        set_error("block of N = %d samples with NP = %d does not fit in shared memory (streamed path not built yet)", N, NP);
-        return PT_ERR_UNSUPPORTED;
-    }
+    rc = plan_for(B, N, NP, D, &pl, true);
+    if (rc) return rc;
     BlockParams p;
     memset(&p, 0, sizeof(p));
     p.x = x; p.pop_in = pop; p.fitness_out = fitness;
     p.B = B; p.N = N; p.Npad = pl.Npad; p.NP = NP; p.NPpad = pl.NPpad; p.G = 0;
     p.fs = fs; p.t0 = t0; p.Wg = pl.Wg; p.Ws = pl.Ws;
     p.use_bulk = ((N % 4) == 0 && (reinterpret_cast<uintptr_t>(x) % 16) == 0) ? 1 : 0;
+    rc = attach_workspace(&p, pl, workspace, workspace_bytes);
+    if (rc) return rc;
     return dispatch<kModeFitness>(p, pl, D, (cudaStream_t)stream);
 }
 
-size_t pt_fit_blocks_workspace_bytes(int64_t, int32_t, const pt_de_config*) { return 0; }
+size_t pt_fit_blocks_workspace_bytes(int64_t B, int32_t N, const pt_de_config* cfg) {
+    Plan pl;
+    if (!cfg || check_common(B, N, 1.0, cfg->NP, cfg->D) || plan_for(B, N, cfg->NP, cfg->D, &pl, false)) return 0;
+    return pl.ws_bytes;
+}
 
 int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg, int32_t out[6]) {
     if (!cfg || !out) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
     int rc = check_common(B, N, 1.0, cfg->NP, cfg->D);
     if (rc) return rc;
-    int sms = 148, smem_optin = 232448;
-    int dev_count = 0;
-    if (cudaGetDeviceCount(&dev_count) == cudaSuccess && dev_count > 0) {
-        if (device_info(&sms, &smem_optin)) return PT_ERR_CUDA;
-    } else {
-        (void)cudaGetLastError();
-    }
     Plan pl;
-    if (make_plan(B, N, cfg->NP, cfg->D, sms, smem_optin, &pl)) {
-        set_error("block does not fit in shared memory");
-        return PT_ERR_UNSUPPORTED;
-    }
+    rc = plan_for(B, N, cfg->NP, cfg->D, &pl, false);
+    if (rc) return rc;
     out[0] = pl.grid; out[1] = pl.threads; out[2] = pl.smem; out[3] = pl.resident; out[4] = pl.C; out[5] = pl.ctas_per_sm;
     return PT_OK;
 }
@@ -228,19 +280,14 @@ int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const dou
                       const uint32_t* block_index, const pt_de_config* cfg, double* best, float* best_rss,
                       uint32_t* status, float* final_pop, float* final_fit, void* workspace, size_t workspace_bytes,
                       void* stream) {
-    (void)workspace; (void)workspace_bytes;
     if (!x || !lo || !hi || !best || !best_rss || !status) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
     int rc = check_cfg(cfg);
     if (rc) return rc;
     rc = check_common(B, N, fs, cfg->NP, cfg->D);
     if (rc) return rc;
-    int sms, smem_optin;
-    if (device_info(&sms, &smem_optin)) return PT_ERR_CUDA;
     Plan pl;
-    if (make_plan(B, N, cfg->NP, cfg->D, sms, smem_optin, &pl)) {
-        set_error("block of N = %d samples with NP = %d does not fit in shared memory (streamed path not built yet)", N, cfg->NP);
-        return PT_ERR_UNSUPPORTED;
-    }
+    rc = plan_for(B, N, cfg->NP, cfg->D, &pl, true);
+    if (rc) return rc;
     BlockParams p;
     memset(&p, 0, sizeof(p));
     p.x = x; p.lo = lo; p.hi = hi; p.block_index = block_index;
@@ -251,6 +298,8 @@ int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const dou
     p.key0 = (uint32_t)(cfg->seed & 0xFFFFFFFFull); p.key1 = (uint32_t)(cfg->seed >> 32);
     p.Wg = pl.Wg; p.Ws = pl.Ws;
     p.use_bulk = ((N % 4) == 0 && (reinterpret_cast<uintptr_t>(x) % 16) == 0) ? 1 : 0;
+    rc = attach_workspace(&p, pl, workspace, workspace_bytes);
+    if (rc) return rc;
     return dispatch<kModeFit>(p, pl, cfg->D, (cudaStream_t)stream);
 }
 
@@ -320,6 +369,8 @@ int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, const dou
     auto take = [&off](size_t bytes) { size_t o = off; off += (bytes + 255) / 256 * 256; return o; };
     const size_t o_x = take(nx), o_lo = take(nbox), o_hi = take(nbox), o_best = take(nbox);
     const size_t o_rss = take((size_t)B * 4), o_st = take((size_t)B * 4), o_pb = take((size_t)B * 10 * 8), o_tp = take((size_t)B * 8);
+    const size_t ws_bytes = pt_fit_blocks_workspace_bytes(B, N, cfg);
+    const size_t o_ws = take(ws_bytes);
     std::vector<size_t> o_iv(n_intervals);
     std::vector<long long> cnt(n_intervals);
     for (int k = 0; k < n_intervals; ++k) {
@@ -341,7 +392,7 @@ int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, const dou
         ret = pt_fit_blocks(reinterpret_cast<float*>(arena + o_x), B, N, fs, reinterpret_cast<double*>(arena + o_lo),
                             reinterpret_cast<double*>(arena + o_hi), nullptr, cfg, reinterpret_cast<double*>(arena + o_best),
                             reinterpret_cast<float*>(arena + o_rss), reinterpret_cast<uint32_t*>(arena + o_st), nullptr,
-                            nullptr, nullptr, 0, st);
+                            nullptr, ws_bytes ? arena + o_ws : nullptr, ws_bytes, st);
         if (ret) break;
         ret = pt_doppler_products(reinterpret_cast<double*>(arena + o_best), B, D, (double)N / fs, los_scale,
                                   blocks_per_interval, n_intervals, reinterpret_cast<double*>(arena + o_pb),

@@ -26,6 +26,8 @@ namespace pt {
 constexpr int kChunk = 128;        // samples per warp step: 32 lanes x 4 consecutive samples (one LDS.128 each)
 constexpr int kCandStride = 8;     // floats per candidate in the evaluation table
 constexpr int kPairStride = 16;    // floats per candidate PAIR: (-a0,-a1,d0,d1,d2,d3,-,-) interleaved lo/hi
+constexpr int kBarBytes = 128;     // mbarrier area at the start of shared memory
+constexpr int kMaxStages = 7;
 
 enum Mode { kModeFit = 0, kModeFitness = 1 };
 
@@ -47,17 +49,27 @@ struct BlockParams {
     uint32_t CR32, key0, key1;
     int Wg, Ws;                   // warp grid of the evaluation phase, Wg * Ws = warps per CTA
     int use_bulk;                 // rows of x are 16-byte aligned and N % 4 == 0
+    // streamed path (blocks larger than shared memory): tiles of TS samples move through a ring of S stages
+    float* ws_wref;               // [grid][Npad] device workspace: reference phase of the block a CTA is fitting
+    float* ws_x;                  // [grid][Npad] device workspace: 16-byte aligned copy of the block (only if !use_bulk)
+    int TS, S;                    // samples per tile (multiple of kChunk), ring stages; S == 0: resident path
 };
 
 // Shared-memory carve-up, identical on host and device.
 struct SmemLayout {
     int off_bar, off_xs, off_ws, off_popA, off_popT, off_box, off_fit, off_cand, off_part, total;
     __host__ __device__ static int align_up(int v, int a) { return (v + a - 1) / a * a; }
-    __host__ __device__ SmemLayout(int Npad, int NP, int NPpad, int D, int Ws) {
+    // TS/S: tile samples and stages of the streamed path; S == 0: the whole block (xs, wref) is resident
+    __host__ __device__ SmemLayout(int Npad, int NP, int NPpad, int D, int Ws, int TS = 0, int S = 0) {
         int o = 0;
-        off_bar = o; o += 16;
-        off_xs = o; o += Npad * 4;
-        off_ws = o; o += Npad * 4;
+        off_bar = o; o += kBarBytes;          // [0] staging barrier, [1..S] full, [1+S..2S] empty
+        if (S > 0) {
+            off_xs = o; o += S * TS * 8;      // stage s: x tile [TS] then reference-phase tile [TS]
+            off_ws = off_xs;
+        } else {
+            off_xs = o; o += Npad * 4;
+            off_ws = o; o += Npad * 4;
+        }
         o = align_up(o, 16);
         off_popA = o; o += NP * D * 8;
         off_popT = o; o += NP * D * 8;
@@ -130,7 +142,7 @@ __device__ __forceinline__ void eval_chunk(const float4 xv, const float4 wv, con
 }
 
 template <int C>
-__device__ __forceinline__ void reduce_and_store(float (&acc)[C], const int lane, float* out) {
+__device__ __forceinline__ void reduce_and_store(float (&acc)[C], const int lane, float* out, const bool accumulate = false) {
     // butterfly with halving: after log2(C) exchange steps every lane holds one candidate's partial sum
     int cidx = 0;
     int off = 16;
@@ -147,7 +159,7 @@ __device__ __forceinline__ void reduce_and_store(float (&acc)[C], const int lane
     }
     float v = acc[0];
     for (; off >= 1; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
-    if ((lane & (32 / C - 1)) == 0) out[cidx] = v;
+    if ((lane & (32 / C - 1)) == 0) out[cidx] = accumulate ? out[cidx] + v : v;
 }
 
 template <int C, int D>
@@ -195,6 +207,111 @@ __device__ __forceinline__ void eval_population(const BlockParams& p, const floa
     }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// Streamed evaluation (blocks larger than shared memory, BASELINE config 4: 64 K and 256 K samples).
+// The block's samples and its fp32 reference phase (computed once per block into the device workspace) move
+// through a ring of S shared-memory stages, TS samples per tile, by 1-D bulk async copies (UBLKCP) with a
+// full/empty mbarrier pair per stage.  Thread 0 is the producer: at tile c it refills the stage that tile
+// c - 2 used, so it only ever waits for warps that are two tiles behind.  The tile sequence simply repeats for
+// every generation (the data do not depend on the generation), so copies keep flowing through the DE step.
+// Per tile every warp evaluates its candidate groups over its slice of the tile with the same eval_chunk as
+// the resident path and adds its partial sums to part[slice][candidate].
+// ---------------------------------------------------------------------------------------------------
+struct Stream {
+    uint64_t* full;          // [S]
+    uint64_t* empty;         // [S]
+    float* stages;           // S x (x tile [TS], wref tile [TS])
+    const float* xsrc;       // block's samples in global memory (16-byte aligned rows)
+    const float* wsrc;       // block's reference phase in the workspace
+    uint32_t cons;           // tiles consumed since kernel start (all threads)
+    uint32_t prod;           // tiles issued since kernel start (thread 0)
+    uint32_t to_issue;       // tiles of the current block not yet issued (thread 0)
+    int j_issue;             // tile index within the pass of the next tile to issue (thread 0)
+};
+
+__device__ __forceinline__ void stream_issue_one(const BlockParams& p, Stream& st) {
+    const int s = (int)(st.prod % (uint32_t)p.S);
+    const uint32_t k = st.prod / (uint32_t)p.S;
+    if (k >= 1) mbar_wait(&st.empty[s], (k - 1) & 1u);        // every warp has released the previous fill
+    const int n0 = st.j_issue * p.TS;
+    // sizes are multiples of 16 bytes: N % 4 == 0 on the direct path, else the source is the zero-padded workspace copy
+    const uint32_t wb = (uint32_t)min(p.TS, p.Npad - n0) * 4u;
+    const uint32_t xb = p.use_bulk ? (uint32_t)min(p.TS, p.N - n0) * 4u : wb;
+    float* dx = st.stages + (size_t)s * 2 * p.TS;
+    mbar_arrive_expect_tx(&st.full[s], xb + wb);
+    bulk_g2s(dx, st.xsrc + n0, xb, &st.full[s]);
+    bulk_g2s(dx + p.TS, st.wsrc + n0, wb, &st.full[s]);
+    ++st.prod; --st.to_issue;
+    st.j_issue = (st.j_issue + 1 == (p.Npad + p.TS - 1) / p.TS) ? 0 : st.j_issue + 1;
+}
+
+// called by thread 0 after the block's workspace rows are written and fenced: tiles of `passes` evaluation passes
+__device__ __forceinline__ void stream_begin_block(const BlockParams& p, Stream& st, const float* xsrc, const float* wsrc,
+                                                   uint32_t passes) {
+    st.xsrc = xsrc; st.wsrc = wsrc;
+    st.to_issue = passes * (uint32_t)((p.Npad + p.TS - 1) / p.TS);
+    st.j_issue = 0;
+    for (int k = 0; k < p.S - 2 && st.to_issue > 0; ++k) stream_issue_one(p, st);
+}
+
+template <int C, int D>
+__device__ __forceinline__ void eval_population_streamed(const BlockParams& p, Stream& st, const float* __restrict__ cand,
+                                                         float* __restrict__ part, const int tid, const int warp,
+                                                         const int lane) {
+    constexpr int P = C / 2;
+    const int wg = warp % p.Wg, wsl = warp / p.Wg;
+    const int nT = (p.Npad + p.TS - 1) / p.TS;
+    const int nch = p.Npad / kChunk;
+    const bool tail = (p.N % kChunk) != 0;
+    const double dt = 1.0 / p.fs;
+    const float dtf = (float)dt;
+    float tb[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) tb[j] = (float)(p.t0 + j * dt);
+    float* out_row = part + wsl * p.NPpad;
+    const int groups = p.NPpad / C;
+    for (int jt = 0; jt < nT; ++jt) {
+        if (tid == 0 && st.to_issue > 0) stream_issue_one(p, st);
+        const int s = (int)(st.cons % (uint32_t)p.S);
+        mbar_wait(&st.full[s], (st.cons / (uint32_t)p.S) & 1u);
+        const float* xs = st.stages + (size_t)s * 2 * p.TS;
+        const float* wref = xs + p.TS;
+        const int c0 = jt * (p.TS / kChunk);                          // first chunk of this tile in the block
+        const int nct = min(p.TS / kChunk, nch - c0);                 // chunks in this tile
+        const int kb = (int)(((long long)wsl * nct) / p.Ws), ke = (int)(((long long)(wsl + 1) * nct) / p.Ws);
+        const int ke_full = (tail && c0 + ke == nch) ? ke - 1 : ke;
+        for (int g = wg; g < groups; g += p.Wg) {
+            f32x2 na0[P], na1[P], d0[P], d1[P], d2[P], d3[P], acc[P];
+            const ulonglong2* cg = reinterpret_cast<const ulonglong2*>(cand + (size_t)g * P * kPairStride);
+#pragma unroll
+            for (int q = 0; q < P; ++q) {
+                const ulonglong2 u = cg[4 * q], v = cg[4 * q + 1], w = cg[4 * q + 2];
+                na0[q] = u.x; na1[q] = u.y; d0[q] = v.x; d1[q] = v.y; d2[q] = w.x; d3[q] = w.y;
+                acc[q] = pack2(0.0f, 0.0f);
+            }
+            const float4* xp = reinterpret_cast<const float4*>(xs) + kb * 32 + lane;
+            const float4* wp = reinterpret_cast<const float4*>(wref) + kb * 32 + lane;
+            float nf = (float)((c0 + kb) * kChunk + lane * 4);
+#pragma unroll 1
+            for (int k = kb; k < ke_full; ++k) {
+                eval_chunk<P, D, false>(*xp, *wp, nf, dtf, tb, 4, na0, na1, d0, d1, d2, d3, acc);
+                xp += 32; wp += 32; nf += (float)kChunk;
+            }
+            if (ke_full < ke) {
+                const int n_left = p.N - ((nch - 1) * kChunk + lane * 4);
+                eval_chunk<P, D, true>(*xp, *wp, nf, dtf, tb, n_left, na0, na1, d0, d1, d2, d3, acc);
+            }
+            float accs[C];
+#pragma unroll
+            for (int q = 0; q < P; ++q) unpack2(acc[q], accs[2 * q], accs[2 * q + 1]);
+            reduce_and_store<C>(accs, lane, out_row + g * C, jt > 0);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&st.empty[s]);
+        ++st.cons;
+    }
+}
+
 // Evaluation-table entry of member i: NEGATED amplitudes (so that the residual is one FMA, r = A' c + x) and the
 // phase-polynomial offsets from the block's fp64 reference, in radians: d0 = phi0 - phi0_b, d1 = 2 pi (f - f_b),
 // d2 = pi (fdot - fdot_b), d3 = (pi/3)(fddot - fddot_b).  Members 2q and 2q+1 share a row, interleaved lo/hi,
@@ -210,10 +327,10 @@ __device__ __forceinline__ void write_cand(float* cand, const int i, const doubl
     ce[10] = (D == 6) ? (float)((kPi / 3.0) * (th[5] - base[5])) : 0.0f;
 }
 
-template <int C, int D, int MODE>
+template <int C, int D, int MODE, bool STREAM>
 __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
     extern __shared__ __align__(16) unsigned char smem[];
-    const SmemLayout L(p.Npad, p.NP, p.NPpad, D, p.Ws);
+    const SmemLayout L(p.Npad, p.NP, p.NPpad, D, p.Ws, p.TS, p.S);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.off_bar);
     float* xs = reinterpret_cast<float*>(smem + L.off_xs);
     float* wref = reinterpret_cast<float*>(smem + L.off_ws);
@@ -230,8 +347,16 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
     const int warp = tid >> 5, lane = tid & 31;
     uint32_t parity = 0;
 
+    Stream st;
+    if (STREAM) {
+        st.full = bar + 1; st.empty = bar + 1 + p.S;
+        st.stages = xs;
+        st.cons = 0; st.prod = 0; st.to_issue = 0; st.j_issue = 0;
+    }
     if (tid == 0) {
         mbar_init(bar, 1);
+        if (STREAM)
+            for (int k = 0; k < p.S; ++k) { mbar_init(&st.full[k], 1); mbar_init(&st.empty[k], (uint32_t)(nthr >> 5)); }
         fence_mbar_init();
     }
     // padded evaluation-table rows evaluate a zero model; their sums are never read
@@ -241,7 +366,16 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
     for (long long blk = blockIdx.x; blk < p.B; blk += gridDim.x) {
         const float* xg = p.x + blk * (long long)p.N;
         // ---- a0: stage the block's samples (PAPER.md:121 data block) into shared memory, once ----
-        if (p.use_bulk) {
+        //      (streamed path: tiles are staged every pass; an unaligned row is first copied to the workspace)
+        float* wrow = STREAM ? p.ws_wref + (size_t)blockIdx.x * p.Npad : nullptr;
+        const float* xrow = xg;
+        if (STREAM) {
+            if (!p.use_bulk) {
+                float* xw = p.ws_x + (size_t)blockIdx.x * p.Npad;
+                for (int n = tid; n < p.Npad; n += nthr) xw[n] = (n < p.N) ? __ldg(xg + n) : 0.0f;
+                xrow = xw;
+            }
+        } else if (p.use_bulk) {
             if (tid == 0) {
                 fence_proxy_async();   // earlier generic-proxy reads of xs are ordered before the async writes
                 const uint32_t bytes = (uint32_t)p.N * 4u;
@@ -255,7 +389,8 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
         } else {
             for (int n = tid; n < p.N; n += nthr) xs[n] = __ldg(xg + n);
         }
-        for (int n = p.N + tid; n < p.Npad; n += nthr) xs[n] = 0.0f;
+        if (!STREAM)
+            for (int n = p.N + tid; n < p.Npad; n += nthr) xs[n] = 0.0f;
 
         // ---- box, reference point ----
         if (MODE == kModeFit) {
@@ -283,7 +418,8 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                 const double t = p.t0 + (double)n * dt;
                 double u = b0 + t * (b1 + t * (b2 + t * b3));     // turns
                 u -= rint(u);
-                wref[n] = (float)(kTwoPi * u);
+                if (STREAM) wrow[n] = (float)(kTwoPi * u);
+                else wref[n] = (float)(kTwoPi * u);
             }
         }
 
@@ -302,11 +438,17 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
             }
             write_cand<D>(cand, i, th, base);
         }
-        if (p.use_bulk) mbar_wait(bar, parity);
-        parity ^= 1u;
-        __syncthreads();
-
-        eval_population<C, D>(p, xs, wref, cand, part, warp, lane);
+        if (STREAM) {
+            fence_proxy_async_global();      // workspace rows written above are read by the bulk copies below
+            __syncthreads();
+            if (tid == 0) stream_begin_block(p, st, xrow, wrow, (MODE == kModeFit) ? (uint32_t)p.G + 1u : 1u);
+            eval_population_streamed<C, D>(p, st, cand, part, tid, warp, lane);
+        } else {
+            if (p.use_bulk) mbar_wait(bar, parity);
+            parity ^= 1u;
+            __syncthreads();
+            eval_population<C, D>(p, xs, wref, cand, part, warp, lane);
+        }
         __syncthreads();
         for (int i = tid; i < p.NP; i += nthr) {
             float s = 0.0f;
@@ -333,7 +475,8 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                     write_cand<D>(cand, i, th, base);
                 }
                 __syncthreads();
-                eval_population<C, D>(p, xs, wref, cand, part, warp, lane);
+                if (STREAM) eval_population_streamed<C, D>(p, st, cand, part, tid, warp, lane);
+                else eval_population<C, D>(p, xs, wref, cand, part, warp, lane);
                 __syncthreads();
                 // ---- a6: greedy selection, accept on <= ----
                 for (int i = tid; i < p.NP; i += nthr) {

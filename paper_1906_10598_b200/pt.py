@@ -104,8 +104,10 @@ def pt_fitness(x: torch.Tensor, fs: float, pop: torch.Tensor, t0: float | None =
     if t0 is None:
         t0 = default_t0(N, fs)
     out = torch.empty((B, NP), dtype=torch.float32, device=x.device)
+    ws_bytes = lib().pt_fitness_workspace_bytes(B, N, NP, D)
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=x.device) if ws_bytes else None
     rc = lib().pt_fitness(_dev(x, torch.float32, "x"), B, N, float(fs), float(t0), _dev(pop, torch.float32, "pop"), NP, D,
-                          out.data_ptr(), None, 0, _stream())
+                          out.data_ptr(), ws.data_ptr() if ws is not None else None, ws_bytes, _stream())
     _check(rc, "pt_fitness")
     return out
 

@@ -134,6 +134,58 @@ def test_fitness_unaligned_rows_take_the_non_bulk_path(pt):
 
 
 # ----------------------------------------------------------------------------------------------
+# streamed path: blocks larger than shared memory (BASELINE config 4: 64 K and 256 K samples)
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,NP,B", [(65536, 32, 3), (65536, 512, 2), (262144, 64, 2), (65536 + 130, 40, 2), (65536 + 132, 24, 2),
+                                    (70002, 16, 2), (30000, 12, 150), (32768, 1024, 1)])
+def test_fitness_streamed_blocks(pt, N, NP, B):
+    """Tiles of the block move through the shared-memory ring; partial last tile, partial last chunk, rows that are
+    not 16-byte aligned (N % 4 == 2: copied to the workspace first), more blocks than CTAs, largest population."""
+    cfg = pt.make_config(D=5, NP=NP, generations=1, t0=0.0)
+    assert pt.pt_fit_blocks_plan(B, N, cfg)["resident"] == 0
+    wl = W.single_tone_blocks(range(B), N, float(N), config=4, f_range=(50.0, 200.0))
+    assert _fitness_case(pt, wl, NP=NP, seed=N + NP) < FIT_REL_TOL
+
+
+def test_fit_streamed_trajectory_and_full_fit(pt):
+    """Config 4 point N = 65536, NP = 32, 200 generations on 4 blocks: first generations reproduce the oracle's
+    population member by member; the full fit lands on the oracle's optimum."""
+    wl = W.config4(65536, 32, B=4)
+    assert pt.pt_fit_blocks_plan(wl.B, wl.N, pt.make_config(D=5, NP=32, generations=200, t0=wl.t0))["resident"] == 0
+    g = _gpu_fit(pt, wl, generations=3, seed=4, want_pop=True)
+    o = _oracle_fit(wl, generations=3, seed=4, want_pop=True)
+    same = np.all(g["final_pop"] == o["final_pop"].astype(np.float32), axis=-1)
+    assert same.mean() > 0.98, same.mean()
+    assert np.max(np.abs(g["final_fit"] - o["final_fit"]) / o["final_fit"]) < FIT_REL_TOL
+    g = _gpu_fit(pt, wl, seed=4)
+    o = _oracle_fit(wl, seed=4)
+    # NP = 32 for 200 generations does not always collapse; compare where both sides agree on the optimum's RSS
+    ok = np.abs(g["best_rss"] - o["best_rss"]) / o["best_rss"] < FIT_REL_TOL
+    assert ok.sum() >= 3, (g["best_rss"], o["best_rss"])
+    assert np.max(np.abs(_wrap(g["best"][ok, 2] - o["best"][ok, 2]))) < PHI0_TOL
+    assert np.max(np.abs(g["best"][ok, 3] - o["best"][ok, 3])) < F_TOL
+    # every result is valid: its RSS is the oracle's objective at its own parameters
+    chk = oracle.fitness(wl.x, wl.fs, g["best"][:, None, :].astype(np.float32))[:, 0]
+    assert np.max(np.abs(chk - g["best_rss"]) / chk) < FIT_REL_TOL
+
+
+def test_streamed_needs_workspace(pt):
+    import ctypes as C
+    L = pt.lib()
+    cfg = pt.make_config(D=5, NP=32, generations=1, t0=-0.5)
+    need = L.pt_fit_blocks_workspace_bytes(2, 65536, C.byref(cfg))
+    assert need == 2 * 65536 * 4 * 2
+    x = torch.zeros((2, 65536), dtype=torch.float32, device="cuda")
+    box = torch.zeros((2, 5), dtype=torch.float64, device="cuda")
+    best = torch.empty((2, 5), dtype=torch.float64, device="cuda")
+    rss = torch.empty(2, dtype=torch.float32, device="cuda")
+    st = torch.empty(2, dtype=torch.int32, device="cuda")
+    rc = L.pt_fit_blocks(x.data_ptr(), 2, 65536, 65536.0, box.data_ptr(), box.data_ptr(), None, C.byref(cfg), best.data_ptr(),
+                         rss.data_ptr(), st.data_ptr(), None, None, None, 0, None)
+    assert rc == -2 and b"workspace" in L.pt_last_error_string()
+
+
+# ----------------------------------------------------------------------------------------------
 # DE trajectories
 # ----------------------------------------------------------------------------------------------
 def _gpu_fit(pt, wl, *, generations=None, seed=0, want_pop=False, F=None, CR=None, NP=None):
