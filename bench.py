@@ -179,6 +179,56 @@ def run_reference(args, rank: int, world: int):
     print(json.dumps(line), flush=True)
 
 
+def run_sweep(args, dev):
+    """BASELINE.json config 4: block length x population sweep, 1024 blocks per launch, D = 5, 200 generations.
+    One JSON line: `points` = fitness evals/s and XU-roofline fraction of every (N, NP); `value` = all points together."""
+    import torch
+    from paper_1906_10598_b200 import pt, workloads as W
+    Ns = [int(v) for v in args.sweep_n.split(",")]
+    NPs = [int(v) for v in args.sweep_np.split(",")]
+    B, G = args.sweep_blocks, args.sweep_generations
+    points, tot_units, tot_ms = [], 0.0, 0.0
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    for N in Ns:
+        wl = W.config4(N, NPs[0], B=B, generations=G)
+        x, lo, hi = (torch.from_numpy(a).to(dev) for a in (wl.x, wl.lo, wl.hi))
+        for NP in NPs:
+            cfg = pt.make_config(D=5, NP=NP, generations=G, F=0.5, CR=0.9, seed=1, t0=wl.t0)
+            plan = pt.pt_fit_blocks_plan(B, N, cfg)
+            for _ in range(max(1, args.warmup if N * NP < 2 ** 22 else 1)):
+                pt.pt_fit_blocks(x, wl.fs, lo, hi, cfg)
+            torch.cuda.synchronize()
+            steps = args.steps if N * NP < 2 ** 24 else 1
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(steps):
+                r = pt.pt_fit_blocks(x, wl.fs, lo, hi, cfg)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / steps
+            units = float(B) * NP * (G + 1) * N
+            rate = units / (ms * 1e-3)
+            tot_units += units
+            tot_ms += ms
+            ok = float((r["best_rss"] > 0).float().mean().item())
+            points.append({"N": N, "NP": NP, "ms": ms, "sample_evals_per_s": rate, "fitness_evals_per_s": rate / N,
+                           "xu_frac": rate / XU_PEAK, "resident": plan["resident"], "threads": plan["threads"],
+                           "ctas_per_sm": plan["ctas_per_sm"], "smem": plan["smem"], "finite": ok})
+        del x
+    clocks = sampler.stop()
+    line = {"metric": METRIC, "value": tot_units / (tot_ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": tot_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "BASELINE.json config 4 (throughput sweep)", "blocks": B, "generations": G, "D": 5,
+                       "N": Ns, "NP": NPs, "l2": "block samples staged once (resident) or streamed from L2/HBM every generation"},
+            "roofline": {"bound": "alu", "peak": XU_PEAK / 1e12, "unit": "T sample-evals/s (1 MUFU cosine each)",
+                         "achieved": tot_units / (tot_ms * 1e-3) / 1e12, "frac": tot_units / (tot_ms * 1e-3) / XU_PEAK,
+                         "traffic": None},
+            "points": points, "clocks": clocks, "gpu_launches": len(points)}
+    print(json.dumps(line), flush=True)
+
+
 def workload_config(name: str, wl, full=True) -> dict:
     return {"workload": "BASELINE.json config 2 (one-hour track)" if name == "config2" else name,
             "blocks": wl.B if full else "%d (sample)" % wl.B, "samples_per_block": wl.N, "fs_hz": wl.fs,
@@ -198,6 +248,10 @@ def main():
     ap.add_argument("--ref-generations", type=int, default=100)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sweep-n", default="1024,4096,16384,65536,262144")
+    ap.add_argument("--sweep-np", default="32,64,128,256,512")
+    ap.add_argument("--sweep-blocks", type=int, default=1024)
+    ap.add_argument("--sweep-generations", type=int, default=200)
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -221,6 +275,11 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     pt.lib()                                              # fail loudly if the CUDA library is missing
+    if args.workload == "sweep":
+        if world > 1:
+            raise SystemExit("--workload sweep is a 1-GPU report")
+        run_sweep(args, dev)
+        return
     wl = make_workload(args.workload, case=rank)          # every rank fits its own track
     cfg = pt.make_config(D=wl.de["D"], NP=wl.de["NP"], generations=wl.de["generations"], F=wl.de["F"], CR=wl.de["CR"],
                          seed=1 + rank, t0=wl.t0)
