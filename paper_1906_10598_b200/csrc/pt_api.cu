@@ -2,6 +2,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <cmath>
 #include <vector>
 
@@ -33,6 +34,7 @@ struct Plan {
     int C, threads, Wg, Ws, ctas_per_sm, grid, smem, Npad, NPpad, resident, sms;
     int TS, S;              // streamed path: samples per tile, ring stages (0, 0 when resident)
     size_t ws_bytes;        // device workspace the launch needs (streamed path only)
+    int K, NpadS;           // cluster path: CTAs per block, padded samples of the largest slice (K = 1: Npad)
 };
 
 static int device_info(int* sms, int* smem_optin) {
@@ -62,7 +64,8 @@ static void choose_warp_grid(int warps, int groups, int nch, int* Wg, int* Ws) {
 }
 
 // sms / smem_optin are passed in so that the plan can also be computed without a device (defaults of B200).
-static int make_plan(long long B, int N, int NP, int D, int sms, int smem_optin, Plan* pl) {
+// force_K > 0 overrides the cluster-size choice (tests, tuning); 0 = automatic
+static int make_plan(long long B, int N, int NP, int D, int sms, int smem_optin, int force_K, Plan* pl) {
     pl->sms = sms;
     pl->C = (NP % 8 == 0) ? 8 : 4;
     pl->NPpad = (NP + pl->C - 1) / pl->C * pl->C;
@@ -70,6 +73,29 @@ static int make_plan(long long B, int N, int NP, int D, int sms, int smem_optin,
     const int groups = pl->NPpad / pl->C, nch = pl->Npad / kChunk;
     const int per_sm_total = smem_optin + 1024;   // 228 KB per SM, 1 KB reserved per resident CTA
     int chosen = 0;
+    pl->K = 1; pl->NpadS = pl->Npad;
+    // Few blocks, many SMs: a thread-block cluster of K CTAs (K SMs) per block, each owning 1/K of the samples.
+    // K = the largest power of two <= min(8, SMs / B) that leaves every CTA at least two chunks of samples.
+    {
+        int K = 1;
+        while (K * 2 <= 8 && (long long)B * (K * 2) <= sms && nch / (K * 2) >= 2) K *= 2;
+        if (force_K > 0) { K = force_K; while (K > 1 && nch / K < 1) K >>= 1; }
+        if (K > 1) {
+            const int threads = 512, warps = threads / 32;
+            const int nchS = (nch + K - 1) / K;
+            int Wg = 1, Ws = warps;
+            choose_warp_grid(warps, groups, nchS, &Wg, &Ws);
+            const SmemLayout L(nchS * kChunk, NP, pl->NPpad, D, Ws, 0, 0, K);
+            if (L.total <= smem_optin) {
+                pl->threads = threads; pl->Wg = Wg; pl->Ws = Ws; pl->ctas_per_sm = 1; pl->smem = L.total;
+                pl->K = K; pl->NpadS = nchS * kChunk;
+                pl->resident = 1; pl->TS = 0; pl->S = 0; pl->ws_bytes = 0;
+                const long long want = (long long)(sms / K) * K;
+                pl->grid = (int)((long long)B * K < want ? (long long)B * K : want);
+                return 0;
+            }
+        }
+    }
     for (int cps = 4; cps >= 1; cps >>= 1) {
         if (cps > 1 && B <= (long long)sms * (cps / 2)) continue;   // not enough blocks to want that many CTAs
         const int threads = 512 / cps, warps = threads / 32;
@@ -104,6 +130,14 @@ static int make_plan(long long B, int N, int NP, int D, int sms, int smem_optin,
     return 0;
 }
 
+// PT_CLUSTER=<K> in the environment forces the cluster size (1 = never cluster); unset/0 = automatic.
+static int force_cluster() {
+    const char* e = getenv("PT_CLUSTER");
+    if (!e || !*e) return 0;
+    const int k = atoi(e);
+    return (k == 1 || k == 2 || k == 4 || k == 8) ? k : 0;
+}
+
 // plan with the current device's limits, or B200's when no device is present (the query entry points)
 static int plan_for(long long B, int N, int NP, int D, Plan* pl, bool need_device) {
     int sms = 148, smem_optin = 232448;
@@ -114,7 +148,7 @@ static int plan_for(long long B, int N, int NP, int D, Plan* pl, bool need_devic
         (void)cudaGetLastError();
         if (need_device) { set_error("no CUDA device"); return PT_ERR_CUDA; }
     }
-    if (make_plan(B, N, NP, D, sms, smem_optin, pl)) {
+    if (make_plan(B, N, NP, D, sms, smem_optin, force_cluster(), pl)) {
         set_error("N = %d with NP = %d: population tables alone exceed shared memory", N, NP);
         return PT_ERR_UNSUPPORTED;
     }
@@ -130,6 +164,30 @@ static int launch_block_kernel(const BlockParams& p, const Plan& pl, cudaStream_
                        "cudaFuncSetAttribute"))
             return PT_ERR_CUDA;
         configured_smem = pl.smem;
+    }
+    if (pl.K > 1) {
+        // one thread-block cluster of K CTAs per data block
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.blockDim = dim3((unsigned)pl.threads);
+        cfg.dynamicSmemBytes = (size_t)pl.smem;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = (unsigned)pl.K; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        int grid = pl.grid;
+        cfg.gridDim = dim3((unsigned)grid);
+        int max_clusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&max_clusters, pt_block_kernel<C, D, MODE, STREAM>, &cfg) == cudaSuccess &&
+            max_clusters > 0 && grid > max_clusters * pl.K)
+            grid = max_clusters * pl.K;       // persistent: no more clusters than can be resident at once
+        else
+            (void)cudaGetLastError();
+        cfg.gridDim = dim3((unsigned)grid);
+        if (check_cuda(cudaLaunchKernelEx(&cfg, pt_block_kernel<C, D, MODE, STREAM>, p), "pt_block_kernel cluster launch"))
+            return PT_ERR_CUDA;
+        return PT_OK;
     }
     pt_block_kernel<C, D, MODE, STREAM><<<pl.grid, pl.threads, pl.smem, st>>>(p);
     if (check_cuda(cudaGetLastError(), "pt_block_kernel launch")) return PT_ERR_CUDA;
@@ -151,6 +209,7 @@ static int dispatch(const BlockParams& p, const Plan& pl, int D, cudaStream_t st
 // streamed path: hand the workspace rows to the kernel
 static int attach_workspace(BlockParams* p, const Plan& pl, void* workspace, size_t workspace_bytes) {
     p->TS = pl.TS; p->S = pl.S;
+    p->K = pl.K; p->NpadS = pl.NpadS;
     if (pl.S == 0) return PT_OK;
     if (!workspace || workspace_bytes < pl.ws_bytes) {
         set_error("streamed path (N = %d does not fit in shared memory) needs %zu bytes of workspace, got %zu", p->N, pl.ws_bytes,
@@ -265,7 +324,7 @@ size_t pt_fit_blocks_workspace_bytes(int64_t B, int32_t N, const pt_de_config* c
     return pl.ws_bytes;
 }
 
-int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg, int32_t out[6]) {
+int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg, int32_t out[8]) {
     if (!cfg || !out) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
     int rc = check_common(B, N, 1.0, cfg->NP, cfg->D);
     if (rc) return rc;
@@ -273,6 +332,7 @@ int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg, int32_
     rc = plan_for(B, N, cfg->NP, cfg->D, &pl, false);
     if (rc) return rc;
     out[0] = pl.grid; out[1] = pl.threads; out[2] = pl.smem; out[3] = pl.resident; out[4] = pl.C; out[5] = pl.ctas_per_sm;
+    out[6] = pl.K; out[7] = 0;
     return PT_OK;
 }
 

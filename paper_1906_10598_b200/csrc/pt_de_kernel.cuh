@@ -53,14 +53,27 @@ struct BlockParams {
     float* ws_wref;               // [grid][Npad] device workspace: reference phase of the block a CTA is fitting
     float* ws_x;                  // [grid][Npad] device workspace: 16-byte aligned copy of the block (only if !use_bulk)
     int TS, S;                    // samples per tile (multiple of kChunk), ring stages; S == 0: resident path
+    // cluster path (few blocks, many SMs): K CTAs of one thread-block cluster fit ONE block together.  CTA r owns the
+    // chunks [r nch / K, (r+1) nch / K) of the block (its own slice of the samples in shared memory), evaluates every
+    // candidate over that slice, and the K partial sums of every candidate are exchanged through distributed shared
+    // memory; the DE step itself is replicated (counter-based RNG, fp64: bit-identical in every CTA).
+    int K;                        // CTAs per cluster = per block; 1: no cluster
+    int NpadS;                    // padded samples of the largest slice (= Npad when K == 1)
+};
+
+// The samples one CTA evaluates: the whole block (K == 1) or its slice of it.
+struct Slice {
+    int N, Npad;                  // valid / padded samples of the slice
+    double t0;                    // time of the slice's first sample relative to the block centre
 };
 
 // Shared-memory carve-up, identical on host and device.
 struct SmemLayout {
-    int off_bar, off_xs, off_ws, off_popA, off_popT, off_box, off_fit, off_cand, off_part, total;
+    int off_bar, off_xs, off_ws, off_popA, off_popT, off_box, off_fit, off_cand, off_part, off_xpart, total;
     __host__ __device__ static int align_up(int v, int a) { return (v + a - 1) / a * a; }
     // TS/S: tile samples and stages of the streamed path; S == 0: the whole block (xs, wref) is resident
-    __host__ __device__ SmemLayout(int Npad, int NP, int NPpad, int D, int Ws, int TS = 0, int S = 0) {
+    // Npad: padded samples this CTA keeps resident (its slice when K > 1); K: CTAs per cluster
+    __host__ __device__ SmemLayout(int Npad, int NP, int NPpad, int D, int Ws, int TS = 0, int S = 0, int K = 1) {
         int o = 0;
         off_bar = o; o += kBarBytes;          // [0] staging barrier, [1..S] full, [1+S..2S] empty
         if (S > 0) {
@@ -78,6 +91,7 @@ struct SmemLayout {
         o = align_up(o, 16);
         off_cand = o; o += NPpad * kCandStride * 4;
         off_part = o; o += Ws * NPpad * 4;
+        off_xpart = o; o += (K > 1) ? 2 * K * NPpad * 4 : 0;     // [2][K][NPpad]: peers' partial sums, double-buffered
         total = align_up(o, 16);
     }
 };
@@ -163,20 +177,20 @@ __device__ __forceinline__ void reduce_and_store(float (&acc)[C], const int lane
 }
 
 template <int C, int D>
-__device__ __forceinline__ void eval_population(const BlockParams& p, const float* __restrict__ xs,
+__device__ __forceinline__ void eval_population(const BlockParams& p, const Slice& sl, const float* __restrict__ xs,
                                                 const float* __restrict__ wref, const float* __restrict__ cand,
                                                 float* __restrict__ part, const int warp, const int lane) {
     constexpr int P = C / 2;
     const int wg = warp % p.Wg, wsl = warp / p.Wg;
-    const int nch = p.Npad / kChunk;
+    const int nch = sl.Npad / kChunk;
     const int kb = (int)(((long long)wsl * nch) / p.Ws), ke = (int)(((long long)(wsl + 1) * nch) / p.Ws);
-    const bool tail = (p.N % kChunk) != 0;             // the last chunk of the block is partial
+    const bool tail = (sl.N % kChunk) != 0;            // the last chunk of the slice is partial
     const int ke_full = (tail && ke == nch) ? ke - 1 : ke;
     const double dt = 1.0 / p.fs;
     const float dtf = (float)dt;
     float tb[4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) tb[j] = (float)(p.t0 + j * dt);
+    for (int j = 0; j < 4; ++j) tb[j] = (float)(sl.t0 + j * dt);
     float* out_row = part + wsl * p.NPpad;
     const int groups = p.NPpad / C;
     for (int g = wg; g < groups; g += p.Wg) {
@@ -191,13 +205,13 @@ __device__ __forceinline__ void eval_population(const BlockParams& p, const floa
         const float4* xp = reinterpret_cast<const float4*>(xs) + kb * 32 + lane;
         const float4* wp = reinterpret_cast<const float4*>(wref) + kb * 32 + lane;
         float nf = (float)(kb * kChunk + lane * 4);
-#pragma unroll 1
+#pragma unroll 2   // two chunks per trip: half as many drain/fill bubbles of the MUFU results (+3 % on config 2)
         for (int k = kb; k < ke_full; ++k) {
             eval_chunk<P, D, false>(*xp, *wp, nf, dtf, tb, 4, na0, na1, d0, d1, d2, d3, acc);
             xp += 32; wp += 32; nf += (float)kChunk;
         }
         if (ke_full < ke) {
-            const int n_left = p.N - ((nch - 1) * kChunk + lane * 4);     // valid samples of this lane (may be <= 0)
+            const int n_left = sl.N - ((nch - 1) * kChunk + lane * 4);    // valid samples of this lane (may be <= 0)
             eval_chunk<P, D, true>(*xp, *wp, nf, dtf, tb, n_left, na0, na1, d0, d1, d2, d3, acc);
         }
         float accs[C];
@@ -330,7 +344,7 @@ __device__ __forceinline__ void write_cand(float* cand, const int i, const doubl
 template <int C, int D, int MODE, bool STREAM>
 __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
     extern __shared__ __align__(16) unsigned char smem[];
-    const SmemLayout L(p.Npad, p.NP, p.NPpad, D, p.Ws, p.TS, p.S);
+    const SmemLayout L(p.NpadS, p.NP, p.NPpad, D, p.Ws, p.TS, p.S, p.K);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.off_bar);
     float* xs = reinterpret_cast<float*>(smem + L.off_xs);
     float* wref = reinterpret_cast<float*>(smem + L.off_ws);
@@ -342,10 +356,28 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
     float* fit = reinterpret_cast<float*>(smem + L.off_fit);
     float* cand = reinterpret_cast<float*>(smem + L.off_cand);
     float* part = reinterpret_cast<float*>(smem + L.off_part);
+    float* xpart = reinterpret_cast<float*>(smem + L.off_xpart);
 
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int warp = tid >> 5, lane = tid & 31;
     uint32_t parity = 0;
+
+    // ---- cluster geometry: CTA `rank` of K owns the chunks [c_lo, c_hi) of every block its cluster fits ----
+    const int K = STREAM ? 1 : p.K;
+    const int rank = (K > 1) ? (int)cluster_ctarank() : 0;
+    const long long first_blk = (K > 1) ? (long long)cluster_id_x() : (long long)blockIdx.x;
+    const long long blk_stride = (long long)gridDim.x / K;
+    Slice sl;
+    int n_lo = 0;
+    {
+        const int nch_blk = p.Npad / kChunk;
+        const int c_lo = (int)(((long long)rank * nch_blk) / K), c_hi = (int)(((long long)(rank + 1) * nch_blk) / K);
+        n_lo = c_lo * kChunk;
+        sl.Npad = (c_hi - c_lo) * kChunk;
+        sl.N = max(0, min(p.N, c_hi * kChunk) - n_lo);
+        sl.t0 = p.t0 + (double)n_lo * (1.0 / p.fs);
+    }
+    uint32_t xchg = 0;             // exchanges of partial sums done so far (selects the xpart buffer)
 
     Stream st;
     if (STREAM) {
@@ -362,9 +394,35 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
     // padded evaluation-table rows evaluate a zero model; their sums are never read
     for (int i = tid; i < p.NPpad * kCandStride; i += nthr) cand[i] = 0.0f;
     __syncthreads();
+    if (K > 1) cluster_sync_all();     // every CTA of the cluster is running before any peer store is issued
 
-    for (long long blk = blockIdx.x; blk < p.B; blk += gridDim.x) {
-        const float* xg = p.x + blk * (long long)p.N;
+    // Sum of the Ws slice partials of member i; with a cluster, the K CTAs' sums are exchanged through distributed
+    // shared memory and added in rank order, so every CTA of the cluster holds the same fp32 value.
+    auto combine_begin = [&]() {
+        if (K > 1) {
+            float* buf = xpart + (size_t)(xchg & 1u) * K * p.NPpad;
+            for (int i = tid; i < p.NP; i += nthr) {
+                float s = 0.0f;
+                for (int w = 0; w < p.Ws; ++w) s += part[w * p.NPpad + i];
+                const float* slot = buf + (size_t)rank * p.NPpad + i;
+                for (int r = 0; r < K; ++r) st_cluster_f32(mapa_shared(slot, (uint32_t)r), s);
+            }
+            cluster_sync_all();
+        }
+    };
+    auto combined = [&](int i) -> float {
+        float s = 0.0f;
+        if (K > 1) {
+            const float* buf = xpart + (size_t)(xchg & 1u) * K * p.NPpad;
+            for (int r = 0; r < K; ++r) s += buf[(size_t)r * p.NPpad + i];
+        } else {
+            for (int w = 0; w < p.Ws; ++w) s += part[w * p.NPpad + i];
+        }
+        return s;
+    };
+
+    for (long long blk = first_blk; blk < p.B; blk += blk_stride) {
+        const float* xg = p.x + blk * (long long)p.N + n_lo;      // this CTA's slice of the block
         // ---- a0: stage the block's samples (PAPER.md:121 data block) into shared memory, once ----
         //      (streamed path: tiles are staged every pass; an unaligned row is first copied to the workspace)
         float* wrow = STREAM ? p.ws_wref + (size_t)blockIdx.x * p.Npad : nullptr;
@@ -378,7 +436,7 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
         } else if (p.use_bulk) {
             if (tid == 0) {
                 fence_proxy_async();   // earlier generic-proxy reads of xs are ordered before the async writes
-                const uint32_t bytes = (uint32_t)p.N * 4u;
+                const uint32_t bytes = (uint32_t)sl.N * 4u;
                 mbar_arrive_expect_tx(bar, bytes);
                 for (uint32_t o = 0; o < bytes; o += 32768u) {
                     const uint32_t len = min(32768u, bytes - o);
@@ -387,10 +445,10 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                 }
             }
         } else {
-            for (int n = tid; n < p.N; n += nthr) xs[n] = __ldg(xg + n);
+            for (int n = tid; n < sl.N; n += nthr) xs[n] = __ldg(xg + n);
         }
         if (!STREAM)
-            for (int n = p.N + tid; n < p.Npad; n += nthr) xs[n] = 0.0f;
+            for (int n = sl.N + tid; n < sl.Npad; n += nthr) xs[n] = 0.0f;
 
         // ---- box, reference point ----
         if (MODE == kModeFit) {
@@ -414,8 +472,9 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
             const double b0 = base[2] * (1.0 / kTwoPi), b1 = base[3], b2 = 0.5 * base[4];
             const double b3 = (D == 6) ? base[5] * (1.0 / 6.0) : 0.0;
             const double dt = 1.0 / p.fs;
-            for (int n = tid; n < p.Npad; n += nthr) {
-                const double t = p.t0 + (double)n * dt;
+            const int nw = STREAM ? p.Npad : sl.Npad;
+            for (int n = tid; n < nw; n += nthr) {
+                const double t = sl.t0 + (double)n * dt;
                 double u = b0 + t * (b1 + t * (b2 + t * b3));     // turns
                 u -= rint(u);
                 if (STREAM) wrow[n] = (float)(kTwoPi * u);
@@ -447,15 +506,16 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
             if (p.use_bulk) mbar_wait(bar, parity);
             parity ^= 1u;
             __syncthreads();
-            eval_population<C, D>(p, xs, wref, cand, part, warp, lane);
+            eval_population<C, D>(p, sl, xs, wref, cand, part, warp, lane);
         }
         __syncthreads();
+        combine_begin();
         for (int i = tid; i < p.NP; i += nthr) {
-            float s = 0.0f;
-            for (int w = 0; w < p.Ws; ++w) s += part[w * p.NPpad + i];
+            const float s = combined(i);
             fit[i] = s;
-            if (MODE == kModeFitness) p.fitness_out[blk * (long long)p.NP + i] = s;
+            if (MODE == kModeFitness && rank == 0) p.fitness_out[blk * (long long)p.NP + i] = s;
         }
+        ++xchg;
         __syncthreads();
 
         if (MODE == kModeFit) {
@@ -476,23 +536,24 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                 }
                 __syncthreads();
                 if (STREAM) eval_population_streamed<C, D>(p, st, cand, part, tid, warp, lane);
-                else eval_population<C, D>(p, xs, wref, cand, part, warp, lane);
+                else eval_population<C, D>(p, sl, xs, wref, cand, part, warp, lane);
                 __syncthreads();
+                combine_begin();
                 // ---- a6: greedy selection, accept on <= ----
                 for (int i = tid; i < p.NP; i += nthr) {
-                    float s = 0.0f;
-                    for (int w = 0; w < p.Ws; ++w) s += part[w * p.NPpad + i];
+                    const float s = combined(i);
                     if (s <= fit[i]) {
                         fit[i] = s;
 #pragma unroll
                         for (int j = 0; j < D; ++j) popA[i * D + j] = popT[i * D + j];
                     }
                 }
+                ++xchg;
                 __syncthreads();
             }
 
-            // ---- a8: best member (lowest index on ties), status, optional final population ----
-            if (warp == 0) {
+            // ---- a8: best member (lowest index on ties), status, optional final population (cluster: CTA 0 writes) ----
+            if (warp == 0 && rank == 0) {
                 float bv = INFINITY, mx = -INFINITY;
                 int bi = 0x7fffffff;
                 for (int i = lane; i < p.NP; i += 32) {
@@ -522,17 +583,19 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                     p.status[blk] = st;
                 }
             }
-            if (p.final_pop) {
+            if (p.final_pop && rank == 0) {
                 float* fp = p.final_pop + blk * (long long)p.NP * D;
                 for (int i = tid; i < p.NP * D; i += nthr) fp[i] = (float)popA[i];
             }
-            if (p.final_fit) {
+            if (p.final_fit && rank == 0) {
                 float* ff = p.final_fit + blk * (long long)p.NP;
                 for (int i = tid; i < p.NP; i += nthr) ff[i] = fit[i];
             }
         }
         __syncthreads();   // xs / popA are reused by the next block of this CTA
     }
+    // no CTA of a cluster exits while a peer may still store into its shared memory
+    if (K > 1) cluster_sync_all();
 }
 
 }  // namespace pt

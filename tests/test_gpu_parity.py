@@ -34,6 +34,33 @@ def _cuda(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
+class _forced_cluster:
+    """PT_CLUSTER=<K> overrides the library's automatic cluster size (include/pt.h, pt_fit_blocks_plan)."""
+
+    def __init__(self, K):
+        self.K = K
+
+    def __enter__(self):
+        import os
+        self.old = os.environ.get("PT_CLUSTER")
+        os.environ["PT_CLUSTER"] = str(self.K)
+
+    def __exit__(self, *a):
+        import os
+        if self.old is None:
+            os.environ.pop("PT_CLUSTER", None)
+        else:
+            os.environ["PT_CLUSTER"] = self.old
+
+
+@pytest.fixture
+def no_cluster():
+    """Few blocks would otherwise be split over a thread-block cluster (and large blocks become resident that way);
+    the streamed-path tests pin the single-CTA plan."""
+    with _forced_cluster(1):
+        yield
+
+
 def _wrap(d):
     return (np.asarray(d) + np.pi) % (2 * np.pi) - np.pi
 
@@ -138,7 +165,7 @@ def test_fitness_unaligned_rows_take_the_non_bulk_path(pt):
 # ----------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("N,NP,B", [(65536, 32, 3), (65536, 512, 2), (262144, 64, 2), (65536 + 130, 40, 2), (65536 + 132, 24, 2),
                                     (70002, 16, 2), (30000, 12, 150), (32768, 1024, 1)])
-def test_fitness_streamed_blocks(pt, N, NP, B):
+def test_fitness_streamed_blocks(pt, no_cluster, N, NP, B):
     """Tiles of the block move through the shared-memory ring; partial last tile, partial last chunk, rows that are
     not 16-byte aligned (N % 4 == 2: copied to the workspace first), more blocks than CTAs, largest population."""
     cfg = pt.make_config(D=5, NP=NP, generations=1, t0=0.0)
@@ -147,7 +174,7 @@ def test_fitness_streamed_blocks(pt, N, NP, B):
     assert _fitness_case(pt, wl, NP=NP, seed=N + NP) < FIT_REL_TOL
 
 
-def test_fit_streamed_trajectory_and_full_fit(pt):
+def test_fit_streamed_trajectory_and_full_fit(pt, no_cluster):
     """Config 4 point N = 65536, NP = 32, 200 generations on 4 blocks: first generations reproduce the oracle's
     population member by member; the full fit lands on the oracle's optimum."""
     wl = W.config4(65536, 32, B=4)
@@ -169,7 +196,7 @@ def test_fit_streamed_trajectory_and_full_fit(pt):
     assert np.max(np.abs(chk - g["best_rss"]) / chk) < FIT_REL_TOL
 
 
-def test_streamed_needs_workspace(pt):
+def test_streamed_needs_workspace(pt, no_cluster):
     import ctypes as C
     L = pt.lib()
     cfg = pt.make_config(D=5, NP=32, generations=1, t0=-0.5)
@@ -183,6 +210,73 @@ def test_streamed_needs_workspace(pt):
     rc = L.pt_fit_blocks(x.data_ptr(), 2, 65536, 65536.0, box.data_ptr(), box.data_ptr(), None, C.byref(cfg), best.data_ptr(),
                          rss.data_ptr(), st.data_ptr(), None, None, None, 0, None)
     assert rc == -2 and b"workspace" in L.pt_last_error_string()
+
+
+# ----------------------------------------------------------------------------------------------
+# cluster path: K CTAs of a thread-block cluster fit one block together
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("K", [1, 2, 4, 8])
+def test_fitness_cluster_sizes(pt, K):
+    """Every cluster size against the oracle: slices of whole chunks, a ragged last slice (config 1: 78 chunks + 16
+    samples), D = 6, NP not a multiple of the register blocking, and blocks with fewer chunks than CTAs."""
+    with _forced_cluster(K):
+        cfg = pt.make_config(D=5, NP=100, generations=1, seed=0, t0=-0.5)
+        assert pt.pt_fit_blocks_plan(3, 10000, cfg)["cluster"] == K
+        assert _fitness_case(pt, W.config1(blocks=[0, 30, 59]), NP=100) < FIT_REL_TOL
+        assert _fitness_case(pt, W.config2(blocks=[5, 3000]), NP=128) < FIT_REL_TOL
+        assert _fitness_case(pt, W.config3(blocks=[17900, 18000]), NP=36) < FIT_REL_TOL
+        assert _fitness_case(pt, W.config0(cases=range(3)), NP=60) < FIT_REL_TOL
+        wl = W.single_tone_blocks(range(2), 130, 130.0, config=4, f_range=(6.5, 26.0))    # 2 chunks: K capped at 2
+        assert _fitness_case(pt, wl, NP=7) < FIT_REL_TOL
+        wl = W.single_tone_blocks(range(2), 1002, 1002.0, config=4, f_range=(50, 200))    # unaligned rows: no bulk copy
+        assert _fitness_case(pt, wl, NP=16) < FIT_REL_TOL
+
+
+def test_cluster_plan_is_automatic_for_few_blocks(pt):
+    cfg = pt.make_config(D=5, NP=100, generations=1000, seed=0, t0=-0.5)
+    big = pt.pt_fit_blocks_plan(4, 65536, cfg)                         # 8 slices of 8192 samples: resident, not streamed
+    assert big["cluster"] == 8 and big["resident"] == 1
+    wl = W.config4(65536, 32, B=4)
+    assert _fitness_case(pt, wl, NP=32, seed=1) < FIT_REL_TOL
+    assert pt.pt_fit_blocks_plan(60, 10000, cfg)["cluster"] == 2       # BASELINE config 1: 60 blocks on 148 SMs
+    assert pt.pt_fit_blocks_plan(1, 10000, cfg)["cluster"] == 8
+    assert pt.pt_fit_blocks_plan(3600, 16000, cfg)["cluster"] == 1
+    assert pt.pt_fit_blocks_plan(1, 256, cfg)["cluster"] == 1          # two chunks: not worth splitting
+
+
+@pytest.mark.parametrize("K", [2, 8])
+def test_fit_cluster_follows_the_oracle(pt, K):
+    """The DE step is replicated in every CTA of the cluster and only partial sums are exchanged: the first generations
+    are the oracle's trajectory member by member, and the full fit lands on the oracle's optimum."""
+    with _forced_cluster(K):
+        wl = W.config1(blocks=[0, 7, 33])
+        g = _gpu_fit(pt, wl, generations=3, seed=9, want_pop=True)
+        o = _oracle_fit(wl, generations=3, seed=9, want_pop=True)
+        same = np.all(g["final_pop"] == o["final_pop"].astype(np.float32), axis=-1)
+        assert same.mean() > 0.98, same.mean()
+        assert np.max(np.abs(g["final_fit"] - o["final_fit"]) / o["final_fit"]) < FIT_REL_TOL
+        wl = W.config0(cases=range(5))
+        g = _gpu_fit(pt, wl, seed=3)
+        o = _oracle_fit(wl, seed=3)
+        _check_fit_vs_oracle_and_truth(wl, g, o)
+
+
+def test_fit_cluster_persistent_loop_and_single_cta_agree(pt):
+    """More blocks than resident clusters (each cluster loops over several blocks) and the same blocks without
+    clusters: same optimum; the sums differ only in fp32 rounding order."""
+    wl = W.config1(blocks=range(40), generations=400)
+    with _forced_cluster(8):
+        a = _gpu_fit(pt, wl, seed=4)
+    with _forced_cluster(1):
+        b = _gpu_fit(pt, wl, seed=4)
+    ok = ((a["status"] & 2) == 0) & ((b["status"] & 2) == 0)         # both populations collapsed
+    assert ok.sum() >= 36, ok.sum()
+    assert np.max(np.abs(a["best_rss"][ok] - b["best_rss"][ok]) / b["best_rss"][ok]) < 1e-5
+    assert np.max(np.abs(_wrap(a["best"][ok, 2] - b["best"][ok, 2]))) < PHI0_TOL
+    assert np.max(np.abs(a["best"][ok, 3] - b["best"][ok, 3])) < F_TOL
+    # every result is valid: its RSS is the oracle's objective at its own parameters
+    chk = oracle.fitness(wl.x, wl.fs, a["best"][:, None, :].astype(np.float32))[:, 0]
+    assert np.max(np.abs(chk - a["best_rss"]) / chk) < FIT_REL_TOL
 
 
 # ----------------------------------------------------------------------------------------------
@@ -341,11 +435,17 @@ def test_fit_config3_blocks(pt):
     o = _oracle_fit(wl, seed=4)
     dphi = _wrap(g["best"][:, 2] - o["best"][:, 2])
     assert np.max(np.abs(dphi)) < PHI0_TOL
-    assert np.max(np.abs(g["best"][:, 3] - o["best"][:, 3])) < F_TOL
+    # DESIGN.md R20: with T = 0.1 s the Cramer-Rao sigma of f is 4.4e-2 Hz and a change of f by 1e-3 Hz moves the RSS
+    # by 1e-7 relative -- one ulp of the fp32 objective (R18) -- so the fp32 and fp64 fits agree on f to a tenth of
+    # the statistical sigma, not to the 1e-3 Hz that north_star quotes for the 1-s blocks.
     T = wl.T
-    inc_g = 2 * np.pi * (g["best"][:, 3] * T + g["best"][:, 5] * T**3 / 24)
-    inc_o = 2 * np.pi * (o["best"][:, 3] * T + o["best"][:, 5] * T**3 / 24)
-    assert np.max(np.abs(inc_g - inc_o)) < 2 * np.pi * F_TOL * T + 1e-6
+    for k in range(wl.B):
+        sig_f = _crlb(wl.truth[k], wl.N, wl.fs, wl.meta["sigma_per_block"][k] if "sigma_per_block" in wl.meta else wl.sigma, 6)[3]
+        f_tol = max(F_TOL, 0.1 * sig_f)
+        assert abs(g["best"][k, 3] - o["best"][k, 3]) < f_tol, (k, f_tol)
+        inc_g = 2 * np.pi * (g["best"][k, 3] * T + g["best"][k, 5] * T**3 / 24)
+        inc_o = 2 * np.pi * (o["best"][k, 3] * T + o["best"][k, 5] * T**3 / 24)
+        assert abs(inc_g - inc_o) < 2 * np.pi * f_tol * T + 1e-6
     assert np.max(np.abs(g["best_rss"] - o["best_rss"]) / o["best_rss"]) < FIT_REL_TOL
 
 
