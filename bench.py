@@ -379,7 +379,10 @@ def main():
             "data": "synthetic", "config": workload_config(args.workload, wl),
             "real_time_factor": wl.B * wl.T * world / (ms_per_step * 1e-3),
             "fitness_evals_per_s": value / wl.N, "fit_ms": fit_ms, "doppler_products_ms": prod_ms, "plan": plan,
-            "roofline": roofline, "clocks": clocks, "gpu_launches": args.steps * (3 + len([m for m in m_int if wl.B // m > 0])),
+            "roofline": roofline, "clocks": clocks,
+            # per step: pt_block_kernel (+ a second, cluster launch for the last partial wave), 2 Doppler kernels (per-block
+            # columns, prefix scan) and one kernel per integration interval
+            "gpu_launches": args.steps * ((2 if plan.get("tail_cluster") else 1) + 2 + len([m for m in m_int if wl.B // m > 0])),
             "peaks_file": _peaks().get("when")}
     if e2e is not None:
         line["e2e"] = e2e

@@ -156,8 +156,9 @@ PT_API int32_t pt_peak_probe(int32_t kind, double* ops_per_s /*[host]*/);
 /* Launch geometry the library would use for pt_fit_blocks (for reporting): out[0] = grid, out[1] = threads per CTA,
  * out[2] = dynamic shared memory bytes, out[3] = 1 if the block's samples stay resident in shared memory, 0 if streamed,
  * out[4] = candidates per thread (register blocking), out[5] = CTAs per SM, out[6] = CTAs per data block (size of the
- * thread-block cluster that fits one block together when there are fewer blocks than SMs; 1 = no cluster), out[7] = 0.
- * The environment variable PT_CLUSTER = 1 | 2 | 4 | 8 overrides the automatic cluster size (tests and tuning). */
+ * thread-block cluster that fits one block together when there are fewer blocks than SMs; 1 = no cluster), out[7] = cluster
+ * size of the second launch that fits the last partial wave of blocks (0 = single launch; needs a device to be known).
+ * The environment variable PT_CLUSTER = 1..8 overrides the automatic cluster size and disables the tail launch (tests and tuning). */
 PT_API int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg /*[host]*/, int32_t out[8] /*[host]*/);
 
 PT_API const char* pt_last_error_string(void);

@@ -79,7 +79,7 @@ static int make_plan(long long B, int N, int NP, int D, int sms, int smem_optin,
     {
         int K = 1;
         while (K * 2 <= 8 && (long long)B * (K * 2) <= sms && nch / (K * 2) >= 2) K *= 2;
-        if (force_K > 0) { K = force_K; while (K > 1 && nch / K < 1) K >>= 1; }
+        if (force_K > 0) { K = force_K; while (K > 1 && nch / K < 1) --K; }
         if (K > 1) {
             const int threads = 512, warps = threads / 32;
             const int nchS = (nch + K - 1) / K;
@@ -135,7 +135,7 @@ static int force_cluster() {
     const char* e = getenv("PT_CLUSTER");
     if (!e || !*e) return 0;
     const int k = atoi(e);
-    return (k == 1 || k == 2 || k == 4 || k == 8) ? k : 0;
+    return (k >= 1 && k <= 8) ? k : 0;
 }
 
 // plan with the current device's limits, or B200's when no device is present (the query entry points)
@@ -155,8 +155,19 @@ static int plan_for(long long B, int N, int NP, int D, Plan* pl, bool need_devic
     return PT_OK;
 }
 
+static void cluster_launch_config(const Plan& pl, int grid, cudaStream_t st, cudaLaunchConfig_t* cfg, cudaLaunchAttribute* attr) {
+    memset(cfg, 0, sizeof(*cfg));
+    cfg->gridDim = dim3((unsigned)grid);
+    cfg->blockDim = dim3((unsigned)pl.threads);
+    cfg->dynamicSmemBytes = (size_t)pl.smem;
+    cfg->stream = st;
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)pl.K; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg->attrs = attr; cfg->numAttrs = 1;
+}
+
 template <int C, int D, int MODE, bool STREAM>
-static int launch_block_kernel(const BlockParams& p, const Plan& pl, cudaStream_t st) {
+static int configure_smem(const Plan& pl) {
     static int configured_smem = -1;
     if (pl.smem > configured_smem) {
         if (check_cuda(cudaFuncSetAttribute(pt_block_kernel<C, D, MODE, STREAM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -165,26 +176,35 @@ static int launch_block_kernel(const BlockParams& p, const Plan& pl, cudaStream_
             return PT_ERR_CUDA;
         configured_smem = pl.smem;
     }
+    return PT_OK;
+}
+
+// clusters of pl.K CTAs that can be resident at once (0 if the query fails)
+template <int C, int D, int MODE, bool STREAM>
+static int max_resident_clusters(const Plan& pl) {
+    if (configure_smem<C, D, MODE, STREAM>(pl)) return 0;
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[1];
+    cluster_launch_config(pl, pl.K, nullptr, &cfg, attr);
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, pt_block_kernel<C, D, MODE, STREAM>, &cfg) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return 0;
+    }
+    return n;
+}
+
+template <int C, int D, int MODE, bool STREAM>
+static int launch_block_kernel(const BlockParams& p, const Plan& pl, cudaStream_t st) {
+    if (configure_smem<C, D, MODE, STREAM>(pl)) return PT_ERR_CUDA;
     if (pl.K > 1) {
         // one thread-block cluster of K CTAs per data block
-        cudaLaunchConfig_t cfg;
-        memset(&cfg, 0, sizeof(cfg));
-        cfg.blockDim = dim3((unsigned)pl.threads);
-        cfg.dynamicSmemBytes = (size_t)pl.smem;
-        cfg.stream = st;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = (unsigned)pl.K; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-        cfg.attrs = attr; cfg.numAttrs = 1;
         int grid = pl.grid;
-        cfg.gridDim = dim3((unsigned)grid);
-        int max_clusters = 0;
-        if (cudaOccupancyMaxActiveClusters(&max_clusters, pt_block_kernel<C, D, MODE, STREAM>, &cfg) == cudaSuccess &&
-            max_clusters > 0 && grid > max_clusters * pl.K)
-            grid = max_clusters * pl.K;       // persistent: no more clusters than can be resident at once
-        else
-            (void)cudaGetLastError();
-        cfg.gridDim = dim3((unsigned)grid);
+        const int max_clusters = max_resident_clusters<C, D, MODE, STREAM>(pl);
+        if (max_clusters > 0 && grid > max_clusters * pl.K) grid = max_clusters * pl.K;   // persistent: resident clusters only
+        cudaLaunchConfig_t cfg;
+        cudaLaunchAttribute attr[1];
+        cluster_launch_config(pl, grid, st, &cfg, attr);
         if (check_cuda(cudaLaunchKernelEx(&cfg, pt_block_kernel<C, D, MODE, STREAM>, p), "pt_block_kernel cluster launch"))
             return PT_ERR_CUDA;
         return PT_OK;
@@ -204,6 +224,29 @@ static int dispatch2(const BlockParams& p, const Plan& pl, int D, cudaStream_t s
 template <int MODE>
 static int dispatch(const BlockParams& p, const Plan& pl, int D, cudaStream_t st) {
     return pl.S > 0 ? dispatch2<MODE, true>(p, pl, D, st) : dispatch2<MODE, false>(p, pl, D, st);
+}
+
+static int fit_max_resident_clusters(const Plan& pl, int D) {
+    if (pl.C == 8) return D == 5 ? max_resident_clusters<8, 5, kModeFit, false>(pl) : max_resident_clusters<8, 6, kModeFit, false>(pl);
+    return D == 5 ? max_resident_clusters<4, 5, kModeFit, false>(pl) : max_resident_clusters<4, 6, kModeFit, false>(pl);
+}
+
+// Tail wave.  B blocks on a persistent grid of `sms` single-CTA blocks take ceil(B / sms) waves; when the last wave
+// is at most half full its `rem` blocks are fitted by a second launch in which a cluster of K = floor(sms / rem)
+// CTAs shares each block, so the tail costs 1/K of a wave.  K is lowered until `rem` clusters are resident at once.
+// Returns the number of tail blocks (0: single launch) and their plan.
+static long long plan_tail(long long B, int N, int NP, int D, const Plan& pl, Plan* tail) {
+    if (force_cluster() != 0 || pl.K != 1 || pl.S != 0 || pl.ctas_per_sm != 1 || B <= pl.sms) return 0;
+    const long long rem = B % pl.sms;
+    if (rem == 0 || rem * 2 > pl.sms) return 0;
+    int sms = 0, smem_optin = 0;
+    if (device_info(&sms, &smem_optin)) return 0;
+    for (int K = (int)(sms / rem) < 8 ? (int)(sms / rem) : 8; K >= 2; --K) {
+        Plan t;
+        if (make_plan(rem, N, NP, D, sms, smem_optin, K, &t) || t.K != K) continue;
+        if (fit_max_resident_clusters(t, D) >= rem) { *tail = t; return rem; }
+    }
+    return 0;
 }
 
 // streamed path: hand the workspace rows to the kernel
@@ -333,6 +376,13 @@ int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg, int32_
     if (rc) return rc;
     out[0] = pl.grid; out[1] = pl.threads; out[2] = pl.smem; out[3] = pl.resident; out[4] = pl.C; out[5] = pl.ctas_per_sm;
     out[6] = pl.K; out[7] = 0;
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) == cudaSuccess && dev_count > 0) {
+        Plan tl;
+        if (plan_tail(B, N, cfg->NP, cfg->D, pl, &tl) > 0) out[7] = tl.K;
+    } else {
+        (void)cudaGetLastError();
+    }
     return PT_OK;
 }
 
@@ -360,7 +410,19 @@ int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const dou
     p.use_bulk = ((N % 4) == 0 && (reinterpret_cast<uintptr_t>(x) % 16) == 0) ? 1 : 0;
     rc = attach_workspace(&p, pl, workspace, workspace_bytes);
     if (rc) return rc;
-    return dispatch<kModeFit>(p, pl, cfg->D, (cudaStream_t)stream);
+    Plan tl;
+    const long long rem = plan_tail(B, N, cfg->NP, cfg->D, pl, &tl);
+    if (rem == 0) return dispatch<kModeFit>(p, pl, cfg->D, (cudaStream_t)stream);
+    // full waves on single CTAs, then the last partial wave on clusters
+    p.B = B - rem;
+    rc = dispatch<kModeFit>(p, pl, cfg->D, (cudaStream_t)stream);
+    if (rc) return rc;
+    BlockParams q = p;
+    q.blk0 = B - rem; q.B = B;
+    q.Wg = tl.Wg; q.Ws = tl.Ws;
+    rc = attach_workspace(&q, tl, nullptr, 0);
+    if (rc) return rc;
+    return dispatch<kModeFit>(q, tl, cfg->D, (cudaStream_t)stream);
 }
 
 int32_t pt_doppler_products(const double* best, int64_t B, int32_t D, double T, double los_scale,

@@ -43,7 +43,8 @@ struct BlockParams {
     uint32_t* status;             // [B]
     float* final_pop;             // [B][NP][D] or null
     float* final_fit;             // [B][NP] or null
-    long long B;
+    long long B;                  // blocks [blk0, B) are fitted by this launch
+    long long blk0;
     int N, Npad, NP, NPpad, G;
     double fs, t0, F;
     uint32_t CR32, key0, key1;
@@ -205,7 +206,7 @@ __device__ __forceinline__ void eval_population(const BlockParams& p, const Slic
         const float4* xp = reinterpret_cast<const float4*>(xs) + kb * 32 + lane;
         const float4* wp = reinterpret_cast<const float4*>(wref) + kb * 32 + lane;
         float nf = (float)(kb * kChunk + lane * 4);
-#pragma unroll 2   // two chunks per trip: half as many drain/fill bubbles of the MUFU results (+3 % on config 2)
+#pragma unroll 4   // four chunks per trip: fewer drain/fill bubbles of the MUFU results (+2 % on config 2)
         for (int k = kb; k < ke_full; ++k) {
             eval_chunk<P, D, false>(*xp, *wp, nf, dtf, tb, 4, na0, na1, d0, d1, d2, d3, acc);
             xp += 32; wp += 32; nf += (float)kChunk;
@@ -421,7 +422,7 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
         return s;
     };
 
-    for (long long blk = first_blk; blk < p.B; blk += blk_stride) {
+    for (long long blk = p.blk0 + first_blk; blk < p.B; blk += blk_stride) {
         const float* xg = p.x + blk * (long long)p.N + n_lo;      // this CTA's slice of the block
         // ---- a0: stage the block's samples (PAPER.md:121 data block) into shared memory, once ----
         //      (streamed path: tiles are staged every pass; an unaligned row is first copied to the workspace)

@@ -146,7 +146,7 @@ def pt_fit_blocks_plan(B: int, N: int, cfg: DEConfig) -> dict:
     out = (C.c_int32 * 8)()
     _check(lib().pt_fit_blocks_plan(B, N, C.byref(cfg), out), "pt_fit_blocks_plan")
     return dict(grid=out[0], threads=out[1], smem=out[2], resident=out[3], cands_per_thread=out[4], ctas_per_sm=out[5],
-                cluster=out[6])
+                cluster=out[6], tail_cluster=out[7])
 
 
 def pt_doppler_products(best: torch.Tensor, T: float, los_scale: float = 0.0, blocks_per_interval=()):

@@ -279,6 +279,34 @@ def test_fit_cluster_persistent_loop_and_single_cta_agree(pt):
     assert np.max(np.abs(chk - a["best_rss"]) / chk) < FIT_REL_TOL
 
 
+def test_tail_wave_is_fitted_by_clusters_and_matches_the_single_launch(pt):
+    """B = SMs + a few blocks: the full wave runs on single CTAs, the remainder on clusters (second launch).  Same
+    blocks with PT_CLUSTER=1 (one launch, no clusters): the Philox streams depend on the block index only, so the
+    first generations are identical populations and the outputs land in the right rows."""
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    B = sms + 5
+    wl = W.config4(2048, 32, B=B, generations=2)
+    cfg = pt.make_config(D=5, NP=32, generations=2, seed=6, t0=wl.t0)
+    plan = pt.pt_fit_blocks_plan(B, 2048, cfg)
+    if plan["ctas_per_sm"] != 1:
+        # small blocks run several CTAs per SM and keep the single launch; use blocks that fill an SM
+        wl = W.config4(16384, 32, B=B, generations=2)
+        cfg = pt.make_config(D=5, NP=32, generations=2, seed=6, t0=wl.t0)
+        plan = pt.pt_fit_blocks_plan(B, 16384, cfg)
+    assert plan["cluster"] == 1 and plan["tail_cluster"] == 8, plan
+    a = _gpu_fit(pt, wl, generations=2, seed=6, want_pop=True)
+    with _forced_cluster(1):
+        b = _gpu_fit(pt, wl, generations=2, seed=6, want_pop=True)
+    same = np.all(a["final_pop"] == b["final_pop"], axis=-1)
+    assert same.mean() > 0.99
+    assert np.max(np.abs(a["final_fit"] - b["final_fit"]) / b["final_fit"]) < 1e-5
+    k = 7          # the 5 tail blocks and the last 2 of the full wave, against the oracle
+    o = oracle.fit_blocks(wl.x[-k:], wl.fs, wl.lo[-k:], wl.hi[-k:], NP=32, generations=2, F=wl.de["F"], CR=wl.de["CR"], seed=6,
+                          block_index=wl.block_index[-k:], want_pop=True)
+    assert np.max(np.abs(a["final_fit"][-k:] - o["final_fit"]) / o["final_fit"]) < FIT_REL_TOL
+    assert (np.all(a["final_pop"][-k:] == o["final_pop"].astype(np.float32), axis=-1)).mean() > 0.98
+
+
 # ----------------------------------------------------------------------------------------------
 # DE trajectories
 # ----------------------------------------------------------------------------------------------
