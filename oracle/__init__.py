@@ -8,11 +8,15 @@ nothing from ``paper_1906_10598_b200`` and shares no code with the CUDA path.
 only compiles it with gcc and marshals numpy arrays into it with ctypes.
 """
 from .pt_oracle import (  # noqa: F401
+    aux_uniforms,
     build,
+    cor,
     cr32,
+    de_trial,
     de_draws,
     default_t0,
     doppler_products,
+    fcor_of_cor,
     fit_blocks,
     fitness,
     indices_from_words,

@@ -13,7 +13,10 @@
  *   - the chi^2 objective with sigma_i = 1,  F = sum_i [s_i - s(c, t_i)]^2           PAPER.md:143-146 (Eq. 4)
  *   - Differential Evolution (random initial population in the parameter box, mutation with a
  *     weighting factor, crossover, selection, fixed iteration count)
- *     as DE/rand/1/bin, step by step as SURVEY 8(c) items 1-6 state it
+ *     as DE/rand/1/bin, step by step as SURVEY 8(c) items 1-6 state it; the other five mutation
+ *     strategies of Table 4's "strategy" item as DESIGN.md reading R21 takes them
+ *   - the correlation objective F_cor = 1 / (arctan(cor(s_i, s(c_k, t_i))) + pi/2) with the
+ *     constant-amplitude model s(t) = A cos(phi(t))                                  PAPER.md:148-155 (Eq. 5-6)
  *   - the Doppler products: phase / frequency at block borders, continuity residuals,
  *     total-count phase, integration Doppler, line-of-sight acceleration             PAPER.md:228-246 (Eq. 7-8),
  *                                                                                    :343-352 (Eq. 16-17), :376-379 (Eq. 19)
@@ -48,6 +51,8 @@ typedef struct {
     double CR;           /* crossover factor CR_XC         */
     uint64_t seed;       /* Philox key                                                   */
     double t0;           /* time of sample 0 relative to the block centre */
+    int32_t strategy;    /* 1..6, Table 4 "strategy"   */
+    int32_t objective;   /* 0: chi^2 (Eq. 4)   1: correlation (Eq. 5-6) */
 } pto_de_config;
 
 int pto_num_threads(void) {
@@ -196,17 +201,134 @@ void pto_fitness(const float* x, int64_t B, int32_t N, double fs, double t0, con
 }
 
 /* ---------------------------------------------------------------------------------------------
- * DE/rand/1/bin on one block.  SURVEY 8(c) items 3-6.
+ * Correlation objective.  PAPER.md:148-155 (Eq. 5-6):
+ *     F_cor(c_k) = 1 / ( arctan[ cor(s_i, s(c_k, t_i)) ] + pi/2 ),   s(t) = A cos(c0 + c1 t + c2 t^2 + c3 t^3).
+ * Reading R22: cor is the plain (un-normalised) correlation sum  cor = sum_i s_i s(c_k, t_i);
+ * only then does F_cor "converge to 1/pi ~ 0.318" -- a normalised coefficient <= 1 would stop
+ * at 1/(pi/4 + pi/2) = 0.424.  A = th[0] (a0, "the average amplitude of signal"); th[1] (a1) is not used.
+ * ------------------------------------------------------------------------------------------- */
+double pto_cor(const float* x, int32_t N, double fs, double t0, const double* th, int32_t D) {
+    double sum = 0.0;
+    for (int32_t n = 0; n < N; ++n) {
+        double t = t0 + (double)n / fs;
+        double s = th[0] * cos(pto_phase(th, D, t));     /* Eq. 6 */
+        sum += (double)x[n] * s;
+    }
+    return sum;
+}
+
+double pto_fcor_of_cor(double cor) { return 1.0 / (atan(cor) + PTO_PI / 2.0); }   /* Eq. 5 */
+
+double pto_fcor(const float* x, int32_t N, double fs, double t0, const double* th, int32_t D) {
+    return pto_fcor_of_cor(pto_cor(x, N, fs, t0, th, D));
+}
+
+/* objective 0: Eq. 4, objective 1: Eq. 5 */
+double pto_objective(const float* x, int32_t N, double fs, double t0, const double* th, int32_t D, int32_t objective) {
+    return objective == 1 ? pto_fcor(x, N, fs, t0, th, D) : pto_rss(x, N, fs, t0, th, D);
+}
+
+/* Objective of given populations, like pto_fitness. */
+void pto_fitness_obj(const float* x, int64_t B, int32_t N, double fs, double t0, const float* pop, int32_t NP,
+                     int32_t D, int32_t objective, double* fitness) {
+    int64_t total = B * (int64_t)NP;
+#pragma omp parallel for schedule(static)
+    for (int64_t k = 0; k < total; ++k) {
+        int64_t b = k / NP;
+        double th[6] = {0, 0, 0, 0, 0, 0};
+        for (int j = 0; j < D; ++j) th[j] = (double)pop[k * D + j];
+        fitness[k] = pto_objective(x + b * (int64_t)N, N, fs, t0, th, D, objective);
+    }
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * Mutation strategies.  PAPER.md:205: "There are six kind of mutation operations strategies in the DE
+ * algorithm [Price et al., 2006]. Among these strategies the third is the best choice for objective
+ * function Eq. 4 and the sixth for Eq. 5"; Table 4 "strategy  3 6".  The paper never
+ * defines them.  Reading R21: the six strategies of Price, Storn & Lampinen (2006), whose
+ * control-parameter names Table 4 mirrors, all with binomial crossover:
+ *   1  DE/rand/1                        v = x_r1 + F (x_r2 - x_r3)
+ *   2  DE/local-to-best/1               v = x_i + F (x_best - x_i) + F (x_r2 - x_r3)
+ *   3  DE/best/1 with jitter            v_j = x_best,j + (x_r2,j - x_r3,j) (F + 0.0001 rand_j)
+ *   4  DE/rand/1, per-vector dither     v = x_r1 + (F + (1 - F) rand_i) (x_r2 - x_r3)
+ *   5  DE/rand/1, per-generation dither v = x_r1 + (F + (1 - F) rand_g) (x_r2 - x_r3)
+ *   6  DE/rand/1 either-or              v = x_r1 + F (x_r2 - x_r3)               if rand_i < 0.5
+ *                                       v = x_r1 + K (x_r2 + x_r3 - 2 x_r1), K = 0.5 (F + 1)   otherwise
+ * x_best = the member with the smallest objective in the population the trials are built from (lowest index
+ * on ties).  Uniform numbers are (word >> 8) 2^-24 of Philox counters (slot, i, g, b): jitter rand_j = slot 3
+ * words 0..3 (j = 0..3) and slot 4 words 0..3 (j = 4..7); rand_i = slot 3 word 0; rand_g = slot 3 word 0 of
+ * candidate index 0xFFFFFFFF.  Indices r1, r2, r3, jrand and the crossover mask are those of SURVEY 8(c) item 3
+ * for every strategy.
+ * ------------------------------------------------------------------------------------------- */
+static double unit_uniform(uint32_t word) { return (double)(word >> 8) * (1.0 / 16777216.0); }
+
+/* the D + 2 auxiliary uniforms of candidate i in generation g: u[0..D-1] jitter, u[8] per-vector, u[9] per-generation */
+void pto_aux_uniforms(uint64_t seed, uint32_t b, uint32_t g, uint32_t i, double u[10]) {
+    uint32_t w3[4], w4[4], wg[4];
+    draw_words(seed, 3u, i, g, b, w3);
+    draw_words(seed, 4u, i, g, b, w4);
+    draw_words(seed, 3u, 0xFFFFFFFFu, g, b, wg);
+    for (int j = 0; j < 4; ++j) { u[j] = unit_uniform(w3[j]); u[4 + j] = unit_uniform(w4[j]); }
+    u[8] = unit_uniform(w3[0]);
+    u[9] = unit_uniform(wg[0]);
+}
+
+/* Trial vector of candidate i in generation g >= 1 of block b, built from the population P[NP][D] of generation
+ * g-1 whose best member is ibest: mutation by cfg->strategy, binomial crossover, reflect-then-clamp bounds. */
+void pto_de_trial(const pto_de_config* cfg, uint32_t b, uint32_t g, uint32_t i, const double* P, int32_t ibest,
+                  const double* lo, const double* hi, double* trial) {
+    const int32_t D = cfg->D, NP = cfg->NP;
+    const double F = cfg->F;
+    int32_t d[5];
+    double u[10];
+    pto_de_draws(cfg->seed, b, g, i, NP, D, pto_cr32(cfg->CR), d);
+    pto_aux_uniforms(cfg->seed, b, g, i, u);
+    const double* xi = P + (int64_t)i * D;
+    const double* x1 = P + (int64_t)d[0] * D;
+    const double* x2 = P + (int64_t)d[1] * D;
+    const double* x3 = P + (int64_t)d[2] * D;
+    const double* xb = P + (int64_t)ibest * D;
+    for (int j = 0; j < D; ++j) {
+        double v;
+        if (!((d[4] >> j) & 1)) { trial[j] = xi[j]; continue; }       /* crossover keeps the parent */
+        switch (cfg->strategy) {
+            case 2: v = (xi[j] + F * (xb[j] - xi[j])) + F * (x2[j] - x3[j]); break;
+            case 3: v = xb[j] + (x2[j] - x3[j]) * (F + 0.0001 * u[j]); break;
+            case 4: v = x1[j] + (F + (1.0 - F) * u[8]) * (x2[j] - x3[j]); break;
+            case 5: v = x1[j] + (F + (1.0 - F) * u[9]) * (x2[j] - x3[j]); break;
+            case 6:
+                if (u[8] < 0.5) v = x1[j] + F * (x2[j] - x3[j]);
+                else v = x1[j] + (0.5 * (F + 1.0)) * ((x2[j] + x3[j]) - 2.0 * x1[j]);
+                break;
+            default: v = x1[j] + F * (x2[j] - x3[j]); break;         /* 1: rand/1 */
+        }
+        /* bound handling: reflect once, then clamp */
+        if (v < lo[j]) v = 2.0 * lo[j] - v;
+        else if (v > hi[j]) v = 2.0 * hi[j] - v;
+        if (v < lo[j]) v = lo[j];
+        if (v > hi[j]) v = hi[j];
+        trial[j] = v;
+    }
+}
+
+static int32_t argmin_lowest(const double* fit, int32_t NP) {
+    int32_t ib = 0;
+    for (int32_t i = 1; i < NP; ++i) if (fit[i] < fit[ib]) ib = i;
+    return ib;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * DE on one block.  SURVEY 8(c) items 3-6; strategy and objective as cfg says.
  * Workspace: pop, trial [NP][D], fit, tfit [NP].  par != 0: spread the NP evaluations of one
  * generation over the host cores (independent; the arithmetic of each is unchanged).
  * ------------------------------------------------------------------------------------------- */
 static void evaluate_all(const float* x, int32_t N, double fs, double t0, const double* P, int32_t NP, int32_t D,
-                         double* out, int par) {
+                         int32_t objective, double* out, int par) {
     if (par) {
 #pragma omp parallel for schedule(static)
-        for (int32_t i = 0; i < NP; ++i) out[i] = pto_rss(x, N, fs, t0, P + (int64_t)i * D, D);
+        for (int32_t i = 0; i < NP; ++i) out[i] = pto_objective(x, N, fs, t0, P + (int64_t)i * D, D, objective);
     } else {
-        for (int32_t i = 0; i < NP; ++i) out[i] = pto_rss(x, N, fs, t0, P + (int64_t)i * D, D);
+        for (int32_t i = 0; i < NP; ++i) out[i] = pto_objective(x, N, fs, t0, P + (int64_t)i * D, D, objective);
     }
 }
 
@@ -214,7 +336,6 @@ static void fit_one_block(const float* x, uint32_t b, int32_t N, double fs, cons
                           const pto_de_config* cfg, double* best, double* best_rss, uint32_t* status,
                           double* final_pop, double* final_fit, double* trace, int par) {
     const int32_t D = cfg->D, NP = cfg->NP, G = cfg->generations;
-    const uint32_t CR32 = pto_cr32(cfg->CR);
     double* pop = (double*)malloc(sizeof(double) * (size_t)NP * D);
     double* trial = (double*)malloc(sizeof(double) * (size_t)NP * D);
     double* fit = (double*)malloc(sizeof(double) * (size_t)NP);
@@ -226,7 +347,7 @@ static void fit_one_block(const float* x, uint32_t b, int32_t N, double fs, cons
         pto_init_uniforms(cfg->seed, b, (uint32_t)i, D, u);
         for (int j = 0; j < D; ++j) pop[(int64_t)i * D + j] = lo[j] + (hi[j] - lo[j]) * u[j];
     }
-    evaluate_all(x, N, fs, cfg->t0, pop, NP, D, fit, par);
+    evaluate_all(x, N, fs, cfg->t0, pop, NP, D, cfg->objective, fit, par);
     if (trace) {
         double m = fit[0];
         for (int32_t i = 1; i < NP; ++i) if (fit[i] < m) m = fit[i];
@@ -234,30 +355,12 @@ static void fit_one_block(const float* x, uint32_t b, int32_t N, double fs, cons
     }
 
     for (int32_t g = 1; g <= G; ++g) {
-        /* all trials of generation g are built from the population of generation g-1 */
-        for (int32_t i = 0; i < NP; ++i) {
-            int32_t d[5];
-            pto_de_draws(cfg->seed, b, (uint32_t)g, (uint32_t)i, NP, D, CR32, d);
-            const double* x1 = pop + (int64_t)d[0] * D;
-            const double* x2 = pop + (int64_t)d[1] * D;
-            const double* x3 = pop + (int64_t)d[2] * D;
-            for (int j = 0; j < D; ++j) {
-                double u;
-                if ((d[4] >> j) & 1) {
-                    u = x1[j] + cfg->F * (x2[j] - x3[j]);          /* mutation rand/1 */
-                    /* bound handling: reflect once, then clamp */
-                    if (u < lo[j]) u = 2.0 * lo[j] - u;
-                    else if (u > hi[j]) u = 2.0 * hi[j] - u;
-                    if (u < lo[j]) u = lo[j];
-                    if (u > hi[j]) u = hi[j];
-                } else {
-                    u = pop[(int64_t)i * D + j];                   /* crossover keeps the parent */
-                }
-                trial[(int64_t)i * D + j] = u;
-            }
-        }
-        evaluate_all(x, N, fs, cfg->t0, trial, NP, D, tfit, par);
-        /* selection: replace if RSS(u) <= RSS(x_i) */
+        /* all trials of generation g are built from the population of generation g-1 (and its best member) */
+        const int32_t ibest = argmin_lowest(fit, NP);
+        for (int32_t i = 0; i < NP; ++i)
+            pto_de_trial(cfg, b, (uint32_t)g, (uint32_t)i, pop, ibest, lo, hi, trial + (int64_t)i * D);
+        evaluate_all(x, N, fs, cfg->t0, trial, NP, D, cfg->objective, tfit, par);
+        /* selection: replace if F_obj(u) <= F_obj(x_i) */
         for (int32_t i = 0; i < NP; ++i) {
             if (tfit[i] <= fit[i]) {
                 fit[i] = tfit[i];
@@ -285,7 +388,11 @@ static void fit_one_block(const float* x, uint32_t b, int32_t N, double fs, cons
         double w = hi[j] - lo[j];
         if (w > 0.0 && (v - lo[j] <= 1e-6 * w || hi[j] - v <= 1e-6 * w)) st |= 1u;
     }
-    if (fmax - fmin > 1e-3 * fmin) st |= 2u;   /* DESIGN.md reading R7: 1e-3, not SURVEY's 1e-6 */
+    /* DESIGN.md reading R7: 1e-3, not SURVEY's 1e-6; for Eq. 5 the spread is taken on F_cor - 1/pi, the quantity
+       the paper displays, which is what tends to zero there */
+    if (cfg->objective == 1) {
+        if (fmax - fmin > 1e-3 * (fmin - 1.0 / PTO_PI)) st |= 2u;
+    } else if (fmax - fmin > 1e-3 * fmin) st |= 2u;
     *best_rss = fmin;
     *status = st;
     if (final_pop) memcpy(final_pop, pop, sizeof(double) * (size_t)NP * D);
@@ -302,6 +409,7 @@ int32_t pto_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const do
                        uint32_t* status, double* final_pop, double* final_fit, double* trace) {
     if (!x || !lo || !hi || !cfg || !best || !best_rss || !status) return -1;
     if (cfg->NP < 4 || (cfg->D != 5 && cfg->D != 6) || cfg->generations < 0 || N < 1 || fs <= 0.0) return -1;
+    if (cfg->strategy < 1 || cfg->strategy > 6 || cfg->objective < 0 || cfg->objective > 1) return -1;
     const int32_t D = cfg->D, NP = cfg->NP, G = cfg->generations;
     int nthreads = pto_num_threads();
     if (B >= nthreads) {

@@ -29,6 +29,8 @@ class _DEConfig(C.Structure):
         ("CR", C.c_double),
         ("seed", C.c_uint64),
         ("t0", C.c_double),
+        ("strategy", C.c_int32),
+        ("objective", C.c_int32),
     ]
 
 
@@ -63,6 +65,13 @@ def _load():
     lib.pto_rss.argtypes = [p, C.c_int32, C.c_double, C.c_double, p, C.c_int32]
     lib.pto_rss.restype = C.c_double
     lib.pto_fitness.argtypes = [p, C.c_int64, C.c_int32, C.c_double, C.c_double, p, C.c_int32, C.c_int32, p]
+    lib.pto_fitness_obj.argtypes = [p, C.c_int64, C.c_int32, C.c_double, C.c_double, p, C.c_int32, C.c_int32, C.c_int32, p]
+    lib.pto_cor.argtypes = [p, C.c_int32, C.c_double, C.c_double, p, C.c_int32]
+    lib.pto_cor.restype = C.c_double
+    lib.pto_fcor_of_cor.argtypes = [C.c_double]
+    lib.pto_fcor_of_cor.restype = C.c_double
+    lib.pto_aux_uniforms.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, p]
+    lib.pto_de_trial.argtypes = [C.POINTER(_DEConfig), C.c_uint32, C.c_uint32, C.c_uint32, p, C.c_int32, p, p, p]
     lib.pto_fit_blocks.argtypes = [p, C.c_int64, C.c_int32, C.c_double, p, p, C.POINTER(_DEConfig), p, p, p, p, p, p, p]
     lib.pto_fit_blocks.restype = C.c_int32
     lib.pto_doppler_products.argtypes = [p, C.c_int64, C.c_int32, C.c_double, C.c_double, p, C.c_int32, p, p, p]
@@ -131,8 +140,42 @@ def rss(x, fs: float, theta, t0: float | None = None) -> float:
     return float(_load().pto_rss(_ptr(x), N, float(fs), float(t0), _ptr(th), int(th.shape[0])))
 
 
-def fitness(x, fs: float, pop, t0: float | None = None):
-    """x[B][N] fp32, pop[B][NP][D] fp32 -> fitness[B][NP] fp64."""
+def cor(x, fs: float, theta, t0: float | None = None) -> float:
+    """Correlation sum of Eq. 5-6 (constant amplitude theta[0])."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    th = np.ascontiguousarray(theta, dtype=np.float64)
+    N = int(x.shape[0])
+    if t0 is None:
+        t0 = default_t0(N, fs)
+    return float(_load().pto_cor(_ptr(x), N, float(fs), float(t0), _ptr(th), int(th.shape[0])))
+
+
+def fcor_of_cor(c: float) -> float:
+    """Eq. 5: 1 / (arctan(cor) + pi/2)."""
+    return float(_load().pto_fcor_of_cor(float(c)))
+
+
+def aux_uniforms(seed: int, b: int, g: int, i: int):
+    """(jitter[8], per-vector, per-generation) uniforms of the strategies 3-6."""
+    u = np.zeros(10, dtype=np.float64)
+    _load().pto_aux_uniforms(int(seed), int(b), int(g), int(i), _ptr(u))
+    return u[:8].copy(), float(u[8]), float(u[9])
+
+
+def de_trial(pop, ibest: int, lo, hi, *, b: int, g: int, i: int, F: float, CR: float, seed: int, strategy: int):
+    """Trial vector of candidate i in generation g built from the population pop[NP][D]."""
+    pop = np.ascontiguousarray(pop, dtype=np.float64)
+    lo = np.ascontiguousarray(lo, dtype=np.float64)
+    hi = np.ascontiguousarray(hi, dtype=np.float64)
+    NP, D = pop.shape
+    cfg = _DEConfig(D, NP, 0, float(F), float(CR), int(seed), 0.0, int(strategy), 0)
+    out = np.zeros(D, dtype=np.float64)
+    _load().pto_de_trial(C.byref(cfg), int(b), int(g), int(i), _ptr(pop), int(ibest), _ptr(lo), _ptr(hi), _ptr(out))
+    return out
+
+
+def fitness(x, fs: float, pop, t0: float | None = None, objective: int = 0):
+    """x[B][N] fp32, pop[B][NP][D] fp32 -> objective[B][NP] fp64 (0: Eq. 4 chi^2, 1: Eq. 5 F_cor)."""
     x = np.ascontiguousarray(x, dtype=np.float32)
     pop = np.ascontiguousarray(pop, dtype=np.float32)
     B, N = x.shape
@@ -141,12 +184,13 @@ def fitness(x, fs: float, pop, t0: float | None = None):
     if t0 is None:
         t0 = default_t0(N, fs)
     out = np.zeros((B, NP), dtype=np.float64)
-    _load().pto_fitness(_ptr(x), B, N, float(fs), float(t0), _ptr(pop), NP, D, _ptr(out))
+    _load().pto_fitness_obj(_ptr(x), B, N, float(fs), float(t0), _ptr(pop), NP, D, int(objective), _ptr(out))
     return out
 
 
 def fit_blocks(x, fs: float, lo, hi, *, NP: int, generations: int, F: float = 0.5, CR: float = 0.9, seed: int = 0,
-               t0: float | None = None, block_index=None, want_pop: bool = False, want_trace: bool = False):
+               t0: float | None = None, block_index=None, want_pop: bool = False, want_trace: bool = False,
+               strategy: int = 1, objective: int = 0):
     """DE fit of every block.  Returns a dict: best[B][D], best_rss[B], status[B] and, on request,
     final_pop[B][NP][D], final_fit[B][NP], trace[B][G+1]."""
     x = np.ascontiguousarray(x, dtype=np.float32)
@@ -157,7 +201,7 @@ def fit_blocks(x, fs: float, lo, hi, *, NP: int, generations: int, F: float = 0.
     assert lo.shape == (B, D) and hi.shape == (B, D)
     if t0 is None:
         t0 = default_t0(N, fs)
-    cfg = _DEConfig(D, int(NP), int(generations), float(F), float(CR), int(seed), float(t0))
+    cfg = _DEConfig(D, int(NP), int(generations), float(F), float(CR), int(seed), float(t0), int(strategy), int(objective))
     best = np.zeros((B, D), dtype=np.float64)
     best_rss = np.zeros(B, dtype=np.float64)
     status = np.zeros(B, dtype=np.uint32)

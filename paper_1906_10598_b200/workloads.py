@@ -105,10 +105,12 @@ def _noise_sigma(a_ref: float, snr_db: float) -> float:
 # Configs 0 and 4: independent single-tone blocks, parameters drawn per block.
 # ------------------------------------------------------------------------------------------
 def single_tone_blocks(cases, N: int, fs: float, *, config: int, snr_db: float = 20.0, box: str = "literal",
-                       noiseless: bool = False, de: dict | None = None, f_range=(50.0, 200.0)) -> Workload:
+                       noiseless: bool = False, de: dict | None = None, f_range=(50.0, 200.0),
+                       a1_zero: bool = False) -> Workload:
     """Block k is drawn from ``default_rng([BASE_SEED + 1000*config + case_k, 0])`` as BASELINE.json config 0
     states: a0~U(0.5,1.5), a1~U(-0.1,0.1), phi0~U(-pi,pi), f~U(50,200) Hz, fdot~U(-1,1) Hz/s; the time axis
-    is t in [-T/2, T/2) about the block centre."""
+    is t in [-T/2, T/2) about the block centre.  ``a1_zero`` sets the amplitude slope to zero after the draw
+    (the constant-amplitude signal of PAPER.md:153, Eq. 6; the other draws are unchanged)."""
     cases = list(cases)
     B = len(cases)
     T = N / fs
@@ -120,6 +122,8 @@ def single_tone_blocks(cases, N: int, fs: float, *, config: int, snr_db: float =
         rng = np.random.default_rng([BASE_SEED + 1000 * config + int(case), 0])
         a0 = rng.uniform(0.5, 1.5)
         a1 = rng.uniform(-0.1, 0.1)
+        if a1_zero:
+            a1 = 0.0
         phi0 = rng.uniform(-np.pi, np.pi)
         f = rng.uniform(*f_range)
         fdot = rng.uniform(-1.0, 1.0)
