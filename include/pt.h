@@ -47,6 +47,33 @@ typedef enum {
 #define PT_MAX_NP 1024      /* population limit of the DE kernel                                  */
 #define PT_PER_BLOCK_COLS 10 /* columns of pt_doppler_products' per_block output                  */
 
+/*
+ * Mutation strategies.  PAPER.md:205: "There are six kind of mutation operations strategies in the DE algorithm
+ * [Price et al., 2006].  Among these strategies the third is the best choice for objective function Eq. 4 and the
+ * sixth for Eq. 5"; Table 4 sets "strategy 3 6".  The paper does not define them; they are taken as
+ * the six strategies of Price, Storn & Lampinen (2006), all with binomial crossover (reading R21).
+ * x_r1, x_r2, x_r3: distinct random members != i; x_best: best member of the previous generation; rand: uniform [0,1).
+ */
+typedef enum {
+    PT_STRATEGY_RAND1 = 1,             /* v = x_r1 + F (x_r2 - x_r3)                                              */
+    PT_STRATEGY_LOCAL_TO_BEST1 = 2,    /* v = x_i + F (x_best - x_i) + F (x_r2 - x_r3)                            */
+    PT_STRATEGY_BEST1_JITTER = 3,      /* v_j = x_best,j + (x_r2,j - x_r3,j) (F + 0.0001 rand_j)                  */
+    PT_STRATEGY_RAND1_VEC_DITHER = 4,  /* v = x_r1 + (F + (1 - F) rand_i) (x_r2 - x_r3), one rand per vector      */
+    PT_STRATEGY_RAND1_GEN_DITHER = 5,  /* same, one rand per generation                                           */
+    PT_STRATEGY_EITHER_OR = 6          /* rand_i < 0.5: as 1; else v = x_r1 + 0.5 (F + 1) (x_r2 + x_r3 - 2 x_r1)  */
+} pt_strategy;
+
+/*
+ * Objectives.  PT_OBJECTIVE_CHI2: Eq. 4, the residual sum of squares of the model of Eq. 2.
+ * PT_OBJECTIVE_COR: Eq. 5, F_cor = 1 / (arctan(cor) + pi/2) with the constant-amplitude model of Eq. 6,
+ * s(t) = a0 cos(phi(t)) (a1 is not used), and cor = sum_n x_n s(t_n), the un-normalised correlation sum (the only
+ * reading under which F_cor "shall converge to 1/pi"; reading R22).  With a free amplitude
+ * this objective diverges: give a0 a zero-width box.  F_cor is strictly decreasing in cor; the
+ * kernel maximises the fp32 correlation sum and reports F_cor - 1/pi (fp64 arithmetic, rounded to fp32), the
+ * quantity the paper displays ("subtracted a constant of 0.31830988618"): it tends to 0 from above.
+ */
+typedef enum { PT_OBJECTIVE_CHI2 = 0, PT_OBJECTIVE_COR = 1 } pt_objective_kind;
+
 /* DE control record: the paper's Table 4 plus the population size it never states. */
 typedef struct {
     int32_t D;           /* 5: (a0,a1,phi0,f,fdot)   6: (+fddot)                     PAPER.md:213 Dim_XC */
@@ -56,6 +83,8 @@ typedef struct {
     double CR;           /* crossover factor CR_XC, in [0, 1]         */
     uint64_t seed;       /* Philox4x32-10 key (low word, high word)                                       */
     double t0;           /* time of sample 0 relative to the block centre [s]; -N/(2 fs) by default       */
+    int32_t strategy;    /* pt_strategy, Table 4 "strategy" (0 is read as PT_STRATEGY_RAND1) */
+    int32_t objective;   /* pt_objective_kind: chi^2 (Eq. 4) or correlation (Eq. 5-6)  */
 } pt_de_config;
 
 /*
@@ -75,22 +104,33 @@ PT_API int32_t pt_fitness(const float* x, int64_t B, int32_t N, double fs, doubl
 
 /*
  * pt_fit_blocks -- Differential Evolution fit of every block (PAPER.md:39-43 Fig. 1, :203-224 Table 4):
- * DE/rand/1/bin, NP members drawn uniformly in the box [lo, hi], then `generations`
- * synchronous generations of mutation v = x_r1 + F (x_r2 - x_r3), binomial crossover with factor CR,
- * reflect-then-clamp bound handling, chi^2 evaluation (Eq. 4) and greedy selection (accept on <=).
+ * NP members drawn uniformly in the box [lo, hi], then `generations` synchronous
+ * generations of mutation by cfg->strategy (default DE/rand/1: v = x_r1 + F (x_r2 - x_r3)), binomial crossover
+ * with factor CR, reflect-then-clamp bound handling, evaluation of cfg->objective (default chi^2, Eq. 4) and
+ * greedy selection (accept on <=).
  * Random numbers are Philox4x32-10 with counter (slot, candidate, generation, block_index) and key = seed,
  * so every draw is independent of any floating-point decision.
  * x            [B][N]     fp32 samples
  * lo, hi       [B][D]     fp64 parameter box per block (XCmin / XCmax); lo == hi is legal
  * block_index  [B]        u32 Philox counter word of each block, or NULL for 0..B-1
  * best         [B][D]     fp64 out: member with the smallest RSS (lowest index on ties)
- * best_rss     [B]        fp32 out: its RSS (the "RSS" column of the paper's output record)
+ * best_rss     [B]        fp32 out: its RSS (the "RSS" column of the paper's output record);
+ *                                   F_cor - 1/pi for PT_OBJECTIVE_COR
  * status       [B]        u32 out: bit0 = best lies within 1e-6 (hi-lo) of a box face;
- *                                  bit1 = population not collapsed (max RSS - min RSS > 1e-3 min RSS)
+ *                                  bit1 = population not collapsed (max RSS - min RSS > 1e-3 min RSS; for the
+ *                                         correlation objective the same rule on F_cor - 1/pi)
  * final_pop    [B][NP][D] fp32 out, optional (NULL): final population rounded to fp32
  * final_fit    [B][NP]    fp32 out, optional (NULL)
  * workspace               >= pt_fit_blocks_workspace_bytes(B, N, cfg) bytes of device scratch (may be NULL if 0)
  */
+/*
+ * pt_objective -- like pt_fitness for either objective: objective = PT_OBJECTIVE_CHI2 writes Eq. 4,
+ * PT_OBJECTIVE_COR writes F_cor - 1/pi of Eq. 5-6 (see pt_objective_kind).  Same arguments otherwise.
+ */
+PT_API int32_t pt_objective(const float* x, int64_t B, int32_t N, double fs, double t0, const float* pop, int32_t NP,
+                     int32_t D, int32_t objective, float* fitness, void* workspace, size_t workspace_bytes,
+                     void* stream);
+
 PT_API size_t pt_fit_blocks_workspace_bytes(int64_t B, int32_t N, const pt_de_config* cfg /*[host]*/);
 PT_API int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const double* lo, const double* hi,
                       const uint32_t* block_index, const pt_de_config* cfg /*[host]*/, double* best,

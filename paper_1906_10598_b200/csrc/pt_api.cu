@@ -166,11 +166,11 @@ static void cluster_launch_config(const Plan& pl, int grid, cudaStream_t st, cud
     cfg->attrs = attr; cfg->numAttrs = 1;
 }
 
-template <int C, int D, int MODE, bool STREAM>
+template <int C, int D, int MODE, bool STREAM, int OBJ>
 static int configure_smem(const Plan& pl) {
     static int configured_smem = -1;
     if (pl.smem > configured_smem) {
-        if (check_cuda(cudaFuncSetAttribute(pt_block_kernel<C, D, MODE, STREAM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        if (check_cuda(cudaFuncSetAttribute(pt_block_kernel<C, D, MODE, STREAM, OBJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             pl.smem),
                        "cudaFuncSetAttribute"))
             return PT_ERR_CUDA;
@@ -180,55 +180,61 @@ static int configure_smem(const Plan& pl) {
 }
 
 // clusters of pl.K CTAs that can be resident at once (0 if the query fails)
-template <int C, int D, int MODE, bool STREAM>
+template <int C, int D, int MODE, bool STREAM, int OBJ>
 static int max_resident_clusters(const Plan& pl) {
-    if (configure_smem<C, D, MODE, STREAM>(pl)) return 0;
+    if (configure_smem<C, D, MODE, STREAM, OBJ>(pl)) return 0;
     cudaLaunchConfig_t cfg;
     cudaLaunchAttribute attr[1];
     cluster_launch_config(pl, pl.K, nullptr, &cfg, attr);
     int n = 0;
-    if (cudaOccupancyMaxActiveClusters(&n, pt_block_kernel<C, D, MODE, STREAM>, &cfg) != cudaSuccess) {
+    if (cudaOccupancyMaxActiveClusters(&n, pt_block_kernel<C, D, MODE, STREAM, OBJ>, &cfg) != cudaSuccess) {
         (void)cudaGetLastError();
         return 0;
     }
     return n;
 }
 
-template <int C, int D, int MODE, bool STREAM>
+template <int C, int D, int MODE, bool STREAM, int OBJ>
 static int launch_block_kernel(const BlockParams& p, const Plan& pl, cudaStream_t st) {
-    if (configure_smem<C, D, MODE, STREAM>(pl)) return PT_ERR_CUDA;
+    if (configure_smem<C, D, MODE, STREAM, OBJ>(pl)) return PT_ERR_CUDA;
     if (pl.K > 1) {
         // one thread-block cluster of K CTAs per data block
         int grid = pl.grid;
-        const int max_clusters = max_resident_clusters<C, D, MODE, STREAM>(pl);
+        const int max_clusters = max_resident_clusters<C, D, MODE, STREAM, OBJ>(pl);
         if (max_clusters > 0 && grid > max_clusters * pl.K) grid = max_clusters * pl.K;   // persistent: resident clusters only
         cudaLaunchConfig_t cfg;
         cudaLaunchAttribute attr[1];
         cluster_launch_config(pl, grid, st, &cfg, attr);
-        if (check_cuda(cudaLaunchKernelEx(&cfg, pt_block_kernel<C, D, MODE, STREAM>, p), "pt_block_kernel cluster launch"))
+        if (check_cuda(cudaLaunchKernelEx(&cfg, pt_block_kernel<C, D, MODE, STREAM, OBJ>, p), "pt_block_kernel cluster launch"))
             return PT_ERR_CUDA;
         return PT_OK;
     }
-    pt_block_kernel<C, D, MODE, STREAM><<<pl.grid, pl.threads, pl.smem, st>>>(p);
+    pt_block_kernel<C, D, MODE, STREAM, OBJ><<<pl.grid, pl.threads, pl.smem, st>>>(p);
     if (check_cuda(cudaGetLastError(), "pt_block_kernel launch")) return PT_ERR_CUDA;
     return PT_OK;
 }
 
-template <int MODE, bool STREAM>
-static int dispatch2(const BlockParams& p, const Plan& pl, int D, cudaStream_t st) {
+template <int MODE, bool STREAM, int OBJ>
+static int dispatch3(const BlockParams& p, const Plan& pl, int D, cudaStream_t st) {
     if (pl.C == 8)
-        return D == 5 ? launch_block_kernel<8, 5, MODE, STREAM>(p, pl, st) : launch_block_kernel<8, 6, MODE, STREAM>(p, pl, st);
-    return D == 5 ? launch_block_kernel<4, 5, MODE, STREAM>(p, pl, st) : launch_block_kernel<4, 6, MODE, STREAM>(p, pl, st);
+        return D == 5 ? launch_block_kernel<8, 5, MODE, STREAM, OBJ>(p, pl, st) : launch_block_kernel<8, 6, MODE, STREAM, OBJ>(p, pl, st);
+    return D == 5 ? launch_block_kernel<4, 5, MODE, STREAM, OBJ>(p, pl, st) : launch_block_kernel<4, 6, MODE, STREAM, OBJ>(p, pl, st);
+}
+
+template <int MODE, bool STREAM>
+static int dispatch2(const BlockParams& p, const Plan& pl, int D, int objective, cudaStream_t st) {
+    return objective == kObjCor ? dispatch3<MODE, STREAM, kObjCor>(p, pl, D, st) : dispatch3<MODE, STREAM, kObjChi2>(p, pl, D, st);
 }
 
 template <int MODE>
-static int dispatch(const BlockParams& p, const Plan& pl, int D, cudaStream_t st) {
-    return pl.S > 0 ? dispatch2<MODE, true>(p, pl, D, st) : dispatch2<MODE, false>(p, pl, D, st);
+static int dispatch(const BlockParams& p, const Plan& pl, int D, int objective, cudaStream_t st) {
+    return pl.S > 0 ? dispatch2<MODE, true>(p, pl, D, objective, st) : dispatch2<MODE, false>(p, pl, D, objective, st);
 }
 
+// the shared-memory footprint, register count and launch bounds do not depend on the objective
 static int fit_max_resident_clusters(const Plan& pl, int D) {
-    if (pl.C == 8) return D == 5 ? max_resident_clusters<8, 5, kModeFit, false>(pl) : max_resident_clusters<8, 6, kModeFit, false>(pl);
-    return D == 5 ? max_resident_clusters<4, 5, kModeFit, false>(pl) : max_resident_clusters<4, 6, kModeFit, false>(pl);
+    if (pl.C == 8) return D == 5 ? max_resident_clusters<8, 5, kModeFit, false, kObjChi2>(pl) : max_resident_clusters<8, 6, kModeFit, false, kObjChi2>(pl);
+    return D == 5 ? max_resident_clusters<4, 5, kModeFit, false, kObjChi2>(pl) : max_resident_clusters<4, 6, kModeFit, false, kObjChi2>(pl);
 }
 
 // Tail wave.  B blocks on a persistent grid of `sms` single-CTA blocks take ceil(B / sms) waves; when the last wave
@@ -288,6 +294,8 @@ static int check_cfg(const pt_de_config* cfg) {
     if (!(cfg->F >= 0.0 && cfg->F <= 2.0)) { set_error("F must be in [0, 2]"); return PT_ERR_INVALID_ARG; }
     if (!(cfg->CR >= 0.0 && cfg->CR <= 1.0)) { set_error("CR must be in [0, 1]"); return PT_ERR_INVALID_ARG; }
     if (!std::isfinite(cfg->t0)) { set_error("t0 must be finite"); return PT_ERR_INVALID_ARG; }
+    if (cfg->strategy < 0 || cfg->strategy > 6) { set_error("strategy must be 1..6 (0 = DE/rand/1), got %d", cfg->strategy); return PT_ERR_INVALID_ARG; }
+    if (cfg->objective != PT_OBJECTIVE_CHI2 && cfg->objective != PT_OBJECTIVE_COR) { set_error("objective must be 0 (chi^2) or 1 (correlation), got %d", cfg->objective); return PT_ERR_INVALID_ARG; }
     return PT_OK;
 }
 
@@ -341,12 +349,13 @@ size_t pt_fitness_workspace_bytes(int64_t B, int32_t N, int32_t NP, int32_t D) {
     return pl.ws_bytes;
 }
 
-int32_t pt_fitness(const float* x, int64_t B, int32_t N, double fs, double t0, const float* pop, int32_t NP, int32_t D,
-                   float* fitness, void* workspace, size_t workspace_bytes, void* stream) {
+int32_t pt_objective(const float* x, int64_t B, int32_t N, double fs, double t0, const float* pop, int32_t NP, int32_t D,
+                     int32_t objective, float* fitness, void* workspace, size_t workspace_bytes, void* stream) {
     if (!x || !pop || !fitness) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
     int rc = check_common(B, N, fs, NP, D);
     if (rc) return rc;
     if (!std::isfinite(t0)) { set_error("t0 must be finite"); return PT_ERR_INVALID_ARG; }
+    if (objective != PT_OBJECTIVE_CHI2 && objective != PT_OBJECTIVE_COR) { set_error("objective must be 0 (chi^2) or 1 (correlation), got %d", objective); return PT_ERR_INVALID_ARG; }
     Plan pl;
     rc = plan_for(B, N, NP, D, &pl, true);
     if (rc) return rc;
@@ -354,11 +363,16 @@ int32_t pt_fitness(const float* x, int64_t B, int32_t N, double fs, double t0, c
     memset(&p, 0, sizeof(p));
     p.x = x; p.pop_in = pop; p.fitness_out = fitness;
     p.B = B; p.N = N; p.Npad = pl.Npad; p.NP = NP; p.NPpad = pl.NPpad; p.G = 0;
-    p.fs = fs; p.t0 = t0; p.Wg = pl.Wg; p.Ws = pl.Ws;
+    p.fs = fs; p.t0 = t0; p.Wg = pl.Wg; p.Ws = pl.Ws; p.strategy = kRand1;
     p.use_bulk = ((N % 4) == 0 && (reinterpret_cast<uintptr_t>(x) % 16) == 0) ? 1 : 0;
     rc = attach_workspace(&p, pl, workspace, workspace_bytes);
     if (rc) return rc;
-    return dispatch<kModeFitness>(p, pl, D, (cudaStream_t)stream);
+    return dispatch<kModeFitness>(p, pl, D, objective, (cudaStream_t)stream);
+}
+
+int32_t pt_fitness(const float* x, int64_t B, int32_t N, double fs, double t0, const float* pop, int32_t NP, int32_t D,
+                   float* fitness, void* workspace, size_t workspace_bytes, void* stream) {
+    return pt_objective(x, B, N, fs, t0, pop, NP, D, PT_OBJECTIVE_CHI2, fitness, workspace, workspace_bytes, stream);
 }
 
 size_t pt_fit_blocks_workspace_bytes(int64_t B, int32_t N, const pt_de_config* cfg) {
@@ -407,22 +421,23 @@ int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const dou
     p.CR32 = cr32_of(cfg->CR);
     p.key0 = (uint32_t)(cfg->seed & 0xFFFFFFFFull); p.key1 = (uint32_t)(cfg->seed >> 32);
     p.Wg = pl.Wg; p.Ws = pl.Ws;
+    p.strategy = cfg->strategy == 0 ? kRand1 : cfg->strategy;
     p.use_bulk = ((N % 4) == 0 && (reinterpret_cast<uintptr_t>(x) % 16) == 0) ? 1 : 0;
     rc = attach_workspace(&p, pl, workspace, workspace_bytes);
     if (rc) return rc;
     Plan tl;
     const long long rem = plan_tail(B, N, cfg->NP, cfg->D, pl, &tl);
-    if (rem == 0) return dispatch<kModeFit>(p, pl, cfg->D, (cudaStream_t)stream);
+    if (rem == 0) return dispatch<kModeFit>(p, pl, cfg->D, cfg->objective, (cudaStream_t)stream);
     // full waves on single CTAs, then the last partial wave on clusters
     p.B = B - rem;
-    rc = dispatch<kModeFit>(p, pl, cfg->D, (cudaStream_t)stream);
+    rc = dispatch<kModeFit>(p, pl, cfg->D, cfg->objective, (cudaStream_t)stream);
     if (rc) return rc;
     BlockParams q = p;
     q.blk0 = B - rem; q.B = B;
     q.Wg = tl.Wg; q.Ws = tl.Ws;
     rc = attach_workspace(&q, tl, nullptr, 0);
     if (rc) return rc;
-    return dispatch<kModeFit>(q, tl, cfg->D, (cudaStream_t)stream);
+    return dispatch<kModeFit>(q, tl, cfg->D, cfg->objective, (cudaStream_t)stream);
 }
 
 int32_t pt_doppler_products(const double* best, int64_t B, int32_t D, double T, double los_scale,

@@ -30,6 +30,10 @@ constexpr int kBarBytes = 128;     // mbarrier area at the start of shared memor
 constexpr int kMaxStages = 7;
 
 enum Mode { kModeFit = 0, kModeFitness = 1 };
+// Objective: chi^2 of Eq. 4 or the correlation objective of Eq. 5-6,
+//     F_cor = 1 / (arctan(cor) + pi/2),  cor = sum_n x_n a0 cos(phi(t_n))       (constant amplitude a0, a1 unused).
+// F_cor is strictly decreasing in cor, so the kernel minimises -cor (fp32) and maps to F_cor only on output.
+enum Objective { kObjChi2 = 0, kObjCor = 1 };
 
 struct BlockParams {
     const float* x;               // [B][N]
@@ -48,6 +52,7 @@ struct BlockParams {
     int N, Npad, NP, NPpad, G;
     double fs, t0, F;
     uint32_t CR32, key0, key1;
+    int strategy;                 // Strategy (pt_device.cuh), 1..6
     int Wg, Ws;                   // warp grid of the evaluation phase, Wg * Ws = warps per CTA
     int use_bulk;                 // rows of x are 16-byte aligned and N % 4 == 0
     // streamed path (blocks larger than shared memory): tiles of TS samples move through a ring of S stages
@@ -123,7 +128,7 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
 // ---------------------------------------------------------------------------------------------------
 // Evaluation of one group of C = 2 P candidates over one chunk: 4 consecutive samples of this lane.
 // ---------------------------------------------------------------------------------------------------
-template <int P, int D, bool MASKED>
+template <int P, int D, bool MASKED, int OBJ>
 __device__ __forceinline__ void eval_chunk(const float4 xv, const float4 wv, const float nf, const float dtf,
                                            const float (&tb)[4], const int n_left, const f32x2 (&na0)[P],
                                            const f32x2 (&na1)[P], const f32x2 (&d0)[P], const f32x2 (&d1)[P],
@@ -148,10 +153,14 @@ __device__ __forceinline__ void eval_chunk(const float4 xv, const float4 wv, con
             float y0, y1;
             unpack2(y, y0, y1);
             const f32x2 cs = pack2(__cosf(y0), __cosf(y1));
-            f32x2 A = fma2(t2, na1[q], na0[q]);
-            if (MASKED && j >= n_left) A = pack2(0.0f, 0.0f);      // padded sample: residual 0 - 0 * c
-            const f32x2 r = fma2(A, cs, x2);
-            acc[q] = fma2(r, r, acc[q]);
+            if (OBJ == kObjCor) {
+                acc[q] = fma2(cs, x2, acc[q]);                     // Eq. 5-6: sum x cos(phi); a padded sample has x = 0
+            } else {
+                f32x2 A = fma2(t2, na1[q], na0[q]);
+                if (MASKED && j >= n_left) A = pack2(0.0f, 0.0f);  // padded sample: residual 0 - 0 * c
+                const f32x2 r = fma2(A, cs, x2);
+                acc[q] = fma2(r, r, acc[q]);
+            }
         }
     }
 }
@@ -177,7 +186,7 @@ __device__ __forceinline__ void reduce_and_store(float (&acc)[C], const int lane
     if ((lane & (32 / C - 1)) == 0) out[cidx] = accumulate ? out[cidx] + v : v;
 }
 
-template <int C, int D>
+template <int C, int D, int OBJ>
 __device__ __forceinline__ void eval_population(const BlockParams& p, const Slice& sl, const float* __restrict__ xs,
                                                 const float* __restrict__ wref, const float* __restrict__ cand,
                                                 float* __restrict__ part, const int warp, const int lane) {
@@ -208,12 +217,12 @@ __device__ __forceinline__ void eval_population(const BlockParams& p, const Slic
         float nf = (float)(kb * kChunk + lane * 4);
 #pragma unroll 4   // four chunks per trip: fewer drain/fill bubbles of the MUFU results (+2 % on config 2)
         for (int k = kb; k < ke_full; ++k) {
-            eval_chunk<P, D, false>(*xp, *wp, nf, dtf, tb, 4, na0, na1, d0, d1, d2, d3, acc);
+            eval_chunk<P, D, false, OBJ>(*xp, *wp, nf, dtf, tb, 4, na0, na1, d0, d1, d2, d3, acc);
             xp += 32; wp += 32; nf += (float)kChunk;
         }
         if (ke_full < ke) {
             const int n_left = sl.N - ((nch - 1) * kChunk + lane * 4);    // valid samples of this lane (may be <= 0)
-            eval_chunk<P, D, true>(*xp, *wp, nf, dtf, tb, n_left, na0, na1, d0, d1, d2, d3, acc);
+            eval_chunk<P, D, true, OBJ>(*xp, *wp, nf, dtf, tb, n_left, na0, na1, d0, d1, d2, d3, acc);
         }
         float accs[C];
 #pragma unroll
@@ -269,7 +278,7 @@ __device__ __forceinline__ void stream_begin_block(const BlockParams& p, Stream&
     for (int k = 0; k < p.S - 2 && st.to_issue > 0; ++k) stream_issue_one(p, st);
 }
 
-template <int C, int D>
+template <int C, int D, int OBJ>
 __device__ __forceinline__ void eval_population_streamed(const BlockParams& p, Stream& st, const float* __restrict__ cand,
                                                          float* __restrict__ part, const int tid, const int warp,
                                                          const int lane) {
@@ -309,12 +318,12 @@ __device__ __forceinline__ void eval_population_streamed(const BlockParams& p, S
             float nf = (float)((c0 + kb) * kChunk + lane * 4);
 #pragma unroll 1
             for (int k = kb; k < ke_full; ++k) {
-                eval_chunk<P, D, false>(*xp, *wp, nf, dtf, tb, 4, na0, na1, d0, d1, d2, d3, acc);
+                eval_chunk<P, D, false, OBJ>(*xp, *wp, nf, dtf, tb, 4, na0, na1, d0, d1, d2, d3, acc);
                 xp += 32; wp += 32; nf += (float)kChunk;
             }
             if (ke_full < ke) {
                 const int n_left = p.N - ((nch - 1) * kChunk + lane * 4);
-                eval_chunk<P, D, true>(*xp, *wp, nf, dtf, tb, n_left, na0, na1, d0, d1, d2, d3, acc);
+                eval_chunk<P, D, true, OBJ>(*xp, *wp, nf, dtf, tb, n_left, na0, na1, d0, d1, d2, d3, acc);
             }
             float accs[C];
 #pragma unroll
@@ -342,7 +351,7 @@ __device__ __forceinline__ void write_cand(float* cand, const int i, const doubl
     ce[10] = (D == 6) ? (float)((kPi / 3.0) * (th[5] - base[5])) : 0.0f;
 }
 
-template <int C, int D, int MODE, bool STREAM>
+template <int C, int D, int MODE, bool STREAM, int OBJ>
 __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
     extern __shared__ __align__(16) unsigned char smem[];
     const SmemLayout L(p.NpadS, p.NP, p.NPpad, D, p.Ws, p.TS, p.S, p.K);
@@ -419,7 +428,32 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
         } else {
             for (int w = 0; w < p.Ws; ++w) s += part[w * p.NPpad + i];
         }
+        // Eq. 5-6: s = sum x cos(phi); the value minimised is -cor = (-a0) s   (first entry of member i's table row)
+        if (OBJ == kObjCor) s *= cand[(size_t)(i >> 1) * kPairStride + (i & 1)];
         return s;
+    };
+    // argmin of fit[0..NP) with the lowest index on ties, and the maximum; every lane of the calling warp gets them
+    auto warp_argmin = [&](float& bv, int& bi, float& mx) {
+        bv = INFINITY; mx = -INFINITY; bi = 0x7fffffff;
+        for (int i = lane; i < p.NP; i += 32) {
+            const float v = fit[i];
+            if (v < bv || (v == bv && i < bi)) { bv = v; bi = i; }
+            mx = fmaxf(mx, v);
+        }
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) {
+            const float ov = __shfl_xor_sync(0xffffffffu, bv, off);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+            const float om = __shfl_xor_sync(0xffffffffu, mx, off);
+            if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+            mx = fmaxf(mx, om);
+        }
+    };
+    // value reported for a minimised fp32 value v: the RSS itself, or F_cor - 1/pi of cor = -v (PAPER.md:161 displays
+    // the correlation objective with the constant 0.31830988618 subtracted), computed in fp64
+    auto reported = [&](float v) -> double {
+        if (OBJ == kObjCor) return 1.0 / (atan(-(double)v) + 0.5 * kPi) - 1.0 / kPi;
+        return (double)v;
     };
 
     for (long long blk = p.blk0 + first_blk; blk < p.B; blk += blk_stride) {
@@ -502,19 +536,19 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
             fence_proxy_async_global();      // workspace rows written above are read by the bulk copies below
             __syncthreads();
             if (tid == 0) stream_begin_block(p, st, xrow, wrow, (MODE == kModeFit) ? (uint32_t)p.G + 1u : 1u);
-            eval_population_streamed<C, D>(p, st, cand, part, tid, warp, lane);
+            eval_population_streamed<C, D, OBJ>(p, st, cand, part, tid, warp, lane);
         } else {
             if (p.use_bulk) mbar_wait(bar, parity);
             parity ^= 1u;
             __syncthreads();
-            eval_population<C, D>(p, sl, xs, wref, cand, part, warp, lane);
+            eval_population<C, D, OBJ>(p, sl, xs, wref, cand, part, warp, lane);
         }
         __syncthreads();
         combine_begin();
         for (int i = tid; i < p.NP; i += nthr) {
             const float s = combined(i);
             fit[i] = s;
-            if (MODE == kModeFitness && rank == 0) p.fitness_out[blk * (long long)p.NP + i] = s;
+            if (MODE == kModeFitness && rank == 0) p.fitness_out[blk * (long long)p.NP + i] = (float)reported(s);
         }
         ++xchg;
         __syncthreads();
@@ -522,22 +556,40 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
         if (MODE == kModeFit) {
             // ---- a2..a7: generations ----
             for (int g = 1; g <= p.G; ++g) {
+                // best member of the population the trials are built from (strategies 2 and 3); every warp finds it
+                int ibest = 0;
+                if (p.strategy == kLocalToBest1 || p.strategy == kBest1Jitter) {
+                    float bv, mx;
+                    warp_argmin(bv, ibest, mx);
+                }
                 for (int i = tid; i < p.NP; i += nthr) {
                     const Draws dr = de_draws<D>((uint32_t)i, (uint32_t)g, bidx, (uint32_t)p.NP, p.CR32, p.key0, p.key1);
                     double th[D];
+                    if (p.strategy == kRand1) {
 #pragma unroll
-                    for (int j = 0; j < D; ++j) {
-                        const double parent = popA[i * D + j];
-                        const double mut = mutate_coord(popA[dr.r1 * D + j], popA[dr.r2 * D + j], popA[dr.r3 * D + j],
-                                                        p.F, lo_s[j], hi_s[j]);
-                        th[j] = ((dr.mask >> j) & 1u) ? mut : parent;
-                        popT[i * D + j] = th[j];
+                        for (int j = 0; j < D; ++j) {
+                            const double parent = popA[i * D + j];
+                            const double mut = mutate_coord(popA[dr.r1 * D + j], popA[dr.r2 * D + j], popA[dr.r3 * D + j],
+                                                            p.F, lo_s[j], hi_s[j]);
+                            th[j] = ((dr.mask >> j) & 1u) ? mut : parent;
+                        }
+                    } else {
+                        const AuxDraws ax = aux_draws<D>(p.strategy, (uint32_t)i, (uint32_t)g, bidx, p.key0, p.key1);
+#pragma unroll
+                        for (int j = 0; j < D; ++j) {
+                            const double parent = popA[i * D + j];
+                            const double v = mutant_coord(p.strategy, parent, popA[dr.r1 * D + j], popA[dr.r2 * D + j],
+                                                          popA[dr.r3 * D + j], popA[ibest * D + j], p.F, ax.jit[j], ax.u);
+                            th[j] = ((dr.mask >> j) & 1u) ? bound_coord(v, lo_s[j], hi_s[j]) : parent;
+                        }
                     }
+#pragma unroll
+                    for (int j = 0; j < D; ++j) popT[i * D + j] = th[j];
                     write_cand<D>(cand, i, th, base);
                 }
                 __syncthreads();
-                if (STREAM) eval_population_streamed<C, D>(p, st, cand, part, tid, warp, lane);
-                else eval_population<C, D>(p, sl, xs, wref, cand, part, warp, lane);
+                if (STREAM) eval_population_streamed<C, D, OBJ>(p, st, cand, part, tid, warp, lane);
+                else eval_population<C, D, OBJ>(p, sl, xs, wref, cand, part, warp, lane);
                 __syncthreads();
                 combine_begin();
                 // ---- a6: greedy selection, accept on <= ----
@@ -555,21 +607,9 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
 
             // ---- a8: best member (lowest index on ties), status, optional final population (cluster: CTA 0 writes) ----
             if (warp == 0 && rank == 0) {
-                float bv = INFINITY, mx = -INFINITY;
-                int bi = 0x7fffffff;
-                for (int i = lane; i < p.NP; i += 32) {
-                    const float v = fit[i];
-                    if (v < bv || (v == bv && i < bi)) { bv = v; bi = i; }
-                    mx = fmaxf(mx, v);
-                }
-#pragma unroll
-                for (int off = 16; off >= 1; off >>= 1) {
-                    const float ov = __shfl_xor_sync(0xffffffffu, bv, off);
-                    const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
-                    const float om = __shfl_xor_sync(0xffffffffu, mx, off);
-                    if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-                    mx = fmaxf(mx, om);
-                }
+                float bv, mx;
+                int bi;
+                warp_argmin(bv, bi, mx);
                 if (lane == 0) {
                     uint32_t st = 0;
 #pragma unroll
@@ -579,8 +619,14 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                         const double w = hi_s[j] - lo_s[j];
                         if (w > 0.0 && (v - lo_s[j] <= 1e-6 * w || hi_s[j] - v <= 1e-6 * w)) st |= 1u;
                     }
-                    if (mx - bv > 1e-3f * bv) st |= 2u;
-                    p.best_rss[blk] = bv;
+                    if (OBJ == kObjCor) {
+                        const double fb = reported(bv), fw = reported(mx);
+                        if (fw - fb > 1e-3 * fb) st |= 2u;
+                        p.best_rss[blk] = (float)fb;
+                    } else {
+                        if (mx - bv > 1e-3f * bv) st |= 2u;
+                        p.best_rss[blk] = bv;
+                    }
                     p.status[blk] = st;
                 }
             }
@@ -590,7 +636,7 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
             }
             if (p.final_fit && rank == 0) {
                 float* ff = p.final_fit + blk * (long long)p.NP;
-                for (int i = tid; i < p.NP; i += nthr) ff[i] = fit[i];
+                for (int i = tid; i < p.NP; i += nthr) ff[i] = (float)reported(fit[i]);
             }
         }
         __syncthreads();   // xs / popA are reused by the next block of this CTA

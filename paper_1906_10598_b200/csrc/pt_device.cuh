@@ -95,15 +95,78 @@ __device__ __forceinline__ void init_member(uint32_t i, uint32_t b, uint32_t k0,
     }
 }
 
-// Mutation + bound handling of one coordinate: v = x1 + F (x2 - x3); reflect once at the
-// violated face, then clamp.
-__device__ __forceinline__ double mutate_coord(double x1, double x2, double x3, double F, double lo, double hi) {
-    double u = __dadd_rn(x1, __dmul_rn(F, __dsub_rn(x2, x3)));
+// Bound handling of one coordinate: reflect once at the violated face, then clamp.
+__device__ __forceinline__ double bound_coord(double u, double lo, double hi) {
     if (u < lo) u = __dsub_rn(__dmul_rn(2.0, lo), u);
     else if (u > hi) u = __dsub_rn(__dmul_rn(2.0, hi), u);
     if (u < lo) u = lo;
     if (u > hi) u = hi;
     return u;
+}
+
+// Mutation + bound handling of one coordinate, DE/rand/1: v = x1 + F (x2 - x3).
+__device__ __forceinline__ double mutate_coord(double x1, double x2, double x3, double F, double lo, double hi) {
+    return bound_coord(__dadd_rn(x1, __dmul_rn(F, __dsub_rn(x2, x3))), lo, hi);
+}
+
+// The other mutation strategies of Table 4's "strategy" item (reading R21: the six
+// strategies of Price, Storn & Lampinen 2006).  Uniform numbers are (word >> 8) 2^-24 of Philox counters
+// (slot, i, g, b): slot 3 words 0..3 and slot 4 words 0..3 = per-coordinate jitter; slot 3 word 0 = per-vector
+// number; slot 3 word 0 of candidate 0xFFFFFFFF = per-generation number.
+enum Strategy {
+    kRand1 = 1,          // v = x1 + F (x2 - x3)
+    kLocalToBest1 = 2,   // v = xi + F (xb - xi) + F (x2 - x3)
+    kBest1Jitter = 3,    // v_j = xb_j + (x2_j - x3_j) (F + 0.0001 rand_j)
+    kRand1VecDither = 4, // v = x1 + (F + (1 - F) rand_i) (x2 - x3)
+    kRand1GenDither = 5, // v = x1 + (F + (1 - F) rand_g) (x2 - x3)
+    kEitherOr = 6        // v = x1 + F (x2 - x3) if rand_i < 0.5 else x1 + 0.5 (F + 1) (x2 + x3 - 2 x1)
+};
+
+__device__ __forceinline__ double unit_uniform(uint32_t w) { return (double)(w >> 8) * (1.0 / 16777216.0); }
+
+struct AuxDraws {
+    double jit[8];     // per-coordinate jitter numbers (strategy 3)
+    double u;          // per-vector (strategies 4, 6) or per-generation (strategy 5) number
+};
+
+template <int D>
+__device__ __forceinline__ AuxDraws aux_draws(int strategy, uint32_t i, uint32_t g, uint32_t b, uint32_t k0, uint32_t k1) {
+    AuxDraws a;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) a.jit[j] = 0.0;
+    a.u = 0.0;
+    if (strategy == kBest1Jitter) {
+        const U4 w3 = draw_words(3u, i, g, b, k0, k1);
+        a.jit[0] = unit_uniform(w3.x); a.jit[1] = unit_uniform(w3.y); a.jit[2] = unit_uniform(w3.z); a.jit[3] = unit_uniform(w3.w);
+        if (D > 4) {
+            const U4 w4 = draw_words(4u, i, g, b, k0, k1);
+            a.jit[4] = unit_uniform(w4.x); a.jit[5] = unit_uniform(w4.y); a.jit[6] = unit_uniform(w4.z); a.jit[7] = unit_uniform(w4.w);
+        }
+    } else if (strategy == kRand1VecDither || strategy == kEitherOr) {
+        a.u = unit_uniform(draw_words(3u, i, g, b, k0, k1).x);
+    } else if (strategy == kRand1GenDither) {
+        a.u = unit_uniform(draw_words(3u, 0xFFFFFFFFu, g, b, k0, k1).x);
+    }
+    return a;
+}
+
+// mutant value of one coordinate before bound handling; every fp64 operation rounds on its own, in this order
+__device__ __forceinline__ double mutant_coord(int strategy, double xi, double x1, double x2, double x3, double xb,
+                                               double F, double jit, double u) {
+    switch (strategy) {
+        case kLocalToBest1:
+            return __dadd_rn(__dadd_rn(xi, __dmul_rn(F, __dsub_rn(xb, xi))), __dmul_rn(F, __dsub_rn(x2, x3)));
+        case kBest1Jitter:
+            return __dadd_rn(xb, __dmul_rn(__dsub_rn(x2, x3), __dadd_rn(F, __dmul_rn(0.0001, jit))));
+        case kRand1VecDither:
+        case kRand1GenDither:
+            return __dadd_rn(x1, __dmul_rn(__dadd_rn(F, __dmul_rn(__dsub_rn(1.0, F), u)), __dsub_rn(x2, x3)));
+        case kEitherOr:
+            if (u < 0.5) return __dadd_rn(x1, __dmul_rn(F, __dsub_rn(x2, x3)));
+            return __dadd_rn(x1, __dmul_rn(__dmul_rn(0.5, __dadd_rn(F, 1.0)), __dsub_rn(__dadd_rn(x2, x3), __dmul_rn(2.0, x1))));
+        default:
+            return __dadd_rn(x1, __dmul_rn(F, __dsub_rn(x2, x3)));
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------

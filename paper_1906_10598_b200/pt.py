@@ -32,6 +32,8 @@ class DEConfig(C.Structure):
         ("CR", C.c_double),
         ("seed", C.c_uint64),
         ("t0", C.c_double),
+        ("strategy", C.c_int32),
+        ("objective", C.c_int32),
     ]
 
 
@@ -51,6 +53,8 @@ def lib():
     L.pt_fitness_workspace_bytes.restype = sz
     L.pt_fitness.argtypes = [p, i64, i32, f64, f64, p, i32, i32, p, p, sz, p]
     L.pt_fitness.restype = i32
+    L.pt_objective.argtypes = [p, i64, i32, f64, f64, p, i32, i32, i32, p, p, sz, p]
+    L.pt_objective.restype = i32
     L.pt_fit_blocks_workspace_bytes.argtypes = [i64, i32, C.POINTER(DEConfig)]
     L.pt_fit_blocks_workspace_bytes.restype = sz
     L.pt_fit_blocks.argtypes = [p, i64, i32, f64, p, p, p, C.POINTER(DEConfig), p, p, p, p, p, p, sz, p]
@@ -90,9 +94,15 @@ def default_t0(N: int, fs: float) -> float:
     return -float(N) / (2.0 * float(fs))
 
 
+STRATEGY_RAND1, STRATEGY_LOCAL_TO_BEST1, STRATEGY_BEST1_JITTER = 1, 2, 3
+STRATEGY_RAND1_VEC_DITHER, STRATEGY_RAND1_GEN_DITHER, STRATEGY_EITHER_OR = 4, 5, 6
+OBJECTIVE_CHI2, OBJECTIVE_COR = 0, 1
+
+
 def make_config(*, D: int, NP: int, generations: int, F: float = 0.5, CR: float = 0.9, seed: int = 0,
-                t0: float) -> DEConfig:
-    return DEConfig(int(D), int(NP), int(generations), float(F), float(CR), int(seed), float(t0))
+                t0: float, strategy: int = STRATEGY_RAND1, objective: int = OBJECTIVE_CHI2) -> DEConfig:
+    return DEConfig(int(D), int(NP), int(generations), float(F), float(CR), int(seed), float(t0), int(strategy),
+                    int(objective))
 
 
 def pt_fitness(x: torch.Tensor, fs: float, pop: torch.Tensor, t0: float | None = None) -> torch.Tensor:
@@ -109,6 +119,23 @@ def pt_fitness(x: torch.Tensor, fs: float, pop: torch.Tensor, t0: float | None =
     rc = lib().pt_fitness(_dev(x, torch.float32, "x"), B, N, float(fs), float(t0), _dev(pop, torch.float32, "pop"), NP, D,
                           out.data_ptr(), ws.data_ptr() if ws is not None else None, ws_bytes, _stream())
     _check(rc, "pt_fitness")
+    return out
+
+
+def pt_objective(x: torch.Tensor, fs: float, pop: torch.Tensor, objective: int, t0: float | None = None) -> torch.Tensor:
+    """[B][NP] fp32: Eq. 4 (objective 0) or F_cor - 1/pi of Eq. 5-6 (objective 1) of pop[B][NP][D] on x[B][N]."""
+    B, N = x.shape
+    _, NP, D = pop.shape
+    if pop.shape[0] != B:
+        raise PtError("pop must be [B][NP][D]")
+    if t0 is None:
+        t0 = default_t0(N, fs)
+    out = torch.empty((B, NP), dtype=torch.float32, device=x.device)
+    ws_bytes = lib().pt_fitness_workspace_bytes(B, N, NP, D)
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=x.device) if ws_bytes else None
+    rc = lib().pt_objective(_dev(x, torch.float32, "x"), B, N, float(fs), float(t0), _dev(pop, torch.float32, "pop"), NP, D,
+                            int(objective), out.data_ptr(), ws.data_ptr() if ws is not None else None, ws_bytes, _stream())
+    _check(rc, "pt_objective")
     return out
 
 
