@@ -62,6 +62,18 @@ def make_workload(name: str, case: int):
     raise SystemExit("unknown workload %s" % name)
 
 
+def apply_variant(wl, strategy: int, objective: str):
+    """--strategy / --objective: the widened rows.  For the correlation objective the amplitude
+    is fixed (Eq. 6): a0 = the profile's amplitude at the block centre, a1 = 0, zero-width boxes."""
+    wl.de["strategy"] = int(strategy)
+    wl.de["objective"] = 1 if objective == "cor" else 0
+    if objective == "cor":
+        wl.lo = wl.lo.copy(); wl.hi = wl.hi.copy()
+        wl.lo[:, 0] = wl.hi[:, 0] = wl.truth[:, 0]
+        wl.lo[:, 1] = wl.hi[:, 1] = 0.0
+    return wl
+
+
 def sample_evals(wl) -> float:
     return float(wl.B) * wl.de["NP"] * (wl.de["generations"] + 1) * wl.N
 
@@ -131,7 +143,8 @@ def cpu_baseline(wl, budget_blocks=None, generations=200) -> dict:
     G = min(generations, wl.de["generations"])
     t0 = time.perf_counter()
     oracle.fit_blocks(wl.x[:nb], wl.fs, wl.lo[:nb], wl.hi[:nb], NP=wl.de["NP"], generations=G, F=wl.de["F"],
-                      CR=wl.de["CR"], seed=1, block_index=wl.block_index[:nb])
+                      CR=wl.de["CR"], seed=1, block_index=wl.block_index[:nb], strategy=wl.de.get("strategy", 1),
+                      objective=wl.de.get("objective", 0))
     dt = time.perf_counter() - t0
     units = float(nb) * wl.de["NP"] * (G + 1) * wl.N
     return {"value": units / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -155,13 +168,14 @@ def run_reference(args, rank: int, world: int):
         wl = W.config2(blocks=range(2), generations=3)
     else:
         wl = W.config2(blocks=range(nb))
+    wl = apply_variant(wl, args.strategy, args.objective)
     G = min(wl.de["generations"], args.ref_generations)
     units = float(wl.B) * wl.de["NP"] * (G + 1) * wl.N
     times = []
     for it in range(args.warmup + args.steps):
         t0 = time.perf_counter()
         res = oracle.fit_blocks(wl.x, wl.fs, wl.lo, wl.hi, NP=wl.de["NP"], generations=G, F=wl.de["F"], CR=wl.de["CR"],
-                                seed=1, block_index=wl.block_index)
+                                seed=1, block_index=wl.block_index, strategy=wl.de["strategy"], objective=wl.de["objective"])
         oracle.doppler_products(res["best"], wl.T, 0.0, [1])
         dt = time.perf_counter() - t0
         if it >= args.warmup:
@@ -231,6 +245,7 @@ def run_sweep(args, dev):
 
 def workload_config(name: str, wl, full=True) -> dict:
     return {"workload": "BASELINE.json config 2 (one-hour track)" if name == "config2" else name,
+            "strategy": wl.de.get("strategy", 1), "objective": "cor (Eq. 5-6)" if wl.de.get("objective", 0) else "chi2 (Eq. 4)",
             "blocks": wl.B if full else "%d (sample)" % wl.B, "samples_per_block": wl.N, "fs_hz": wl.fs,
             "NP": wl.de["NP"], "D": wl.de["D"], "generations": wl.de["generations"], "F": wl.de["F"], "CR": wl.de["CR"],
             "box": "literal +-20% around the analytic profile", "l2": "inputs_exceed_l2" if wl.x.nbytes > 126e6 else
@@ -246,6 +261,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--ref-generations", type=int, default=100)
+    ap.add_argument("--strategy", type=int, default=1, help="mutation strategy 1..6 (Table 4; default DE/rand/1)")
+    ap.add_argument("--objective", default="chi2", choices=["chi2", "cor"], help="Eq. 4 (default) or Eq. 5-6")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--sweep-n", default="1024,4096,16384,65536,262144")
@@ -280,9 +297,9 @@ def main():
             raise SystemExit("--workload sweep is a 1-GPU report")
         run_sweep(args, dev)
         return
-    wl = make_workload(args.workload, case=rank)          # every rank fits its own track
+    wl = apply_variant(make_workload(args.workload, case=rank), args.strategy, args.objective)   # every rank fits its own track
     cfg = pt.make_config(D=wl.de["D"], NP=wl.de["NP"], generations=wl.de["generations"], F=wl.de["F"], CR=wl.de["CR"],
-                         seed=1 + rank, t0=wl.t0)
+                         seed=1 + rank, t0=wl.t0, strategy=wl.de["strategy"], objective=wl.de["objective"])
     plan = pt.pt_fit_blocks_plan(wl.B, wl.N, cfg)
     m_int = [max(1, int(round(tc / wl.T))) for tc in (1.0, 10.0, 60.0)]
     x_h = torch.from_numpy(wl.x).pin_memory()
@@ -362,12 +379,15 @@ def main():
     achieved = units / (fit_ms * 1e-3)
     sm_mhz = clocks.get("sm_mhz") or SM_MAX_MHZ
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": XU_PEAK / 1e12, "unit": "T sample-evals/s (1 MUFU cosine each)",
-                "frac": achieved / XU_PEAK, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.workload),
-                "kernel": "pt_block_kernel<C=%d,D=%d,fit>" % (plan["cands_per_thread"], wl.de["D"]),
+                "frac": achieved / XU_PEAK,
+                "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.workload) if not wl.de["objective"] else None,
+                "kernel": "pt_block_kernel<C=%d,D=%d,fit,%s>" % (plan["cands_per_thread"], wl.de["D"],
+                                                                "cor" if wl.de["objective"] else "chi2"),
                 "kernel_ms": fit_ms, "peak_source": "derived: 148 SMs x 16 MUFU lanes x 1965 MHz (DESIGN.md); "
                 "MEASURED_PEAKS.json holds no ALU peak",
                 "frac_at_sampled_clock": achieved / (SM_COUNT * XU_LANES_PER_SM * sm_mhz * 1e6),
-                "fp32_flops_achieved_tflops": achieved * (10 if wl.de["D"] == 5 else 12) / 1e12}
+                # algorithmic flops per sample-evaluation: chi^2 5 (D=5) / 6 FMA; correlation 3 / 4 FMA
+                "fp32_flops_achieved_tflops": achieved * ((10 if wl.de["D"] == 5 else 12) - (4 if wl.de["objective"] else 0)) / 1e12}
     try:
         roofline["measured_mufu_peak"] = pt.pt_peak_probe(1) / 1e12
         roofline["measured_ffma_peak_tflops"] = 2 * pt.pt_peak_probe(0) / 1e12
