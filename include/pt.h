@@ -138,6 +138,40 @@ PT_API int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, co
                       size_t workspace_bytes, void* stream);
 
 /*
+ * Quantised samples.  PAPER.md:104-117 (Table 3): the receiver records 8- or 16-bit samples in its narrow-band modes and
+ * 1-, 2-, 4- or 8-bit samples in its wide-band modes; "s_i is the quantized signal value".  The paper gives
+ * no packing or level table; this library takes (reading R23): sample n of a block is the bits-wide field n of
+ * the block's row, fields packed from the least significant bit of each byte upwards, 16-bit samples little-endian; the
+ * field is an unsigned integer (is_signed = 0) or two's complement (is_signed != 0); the sample value is
+ *     s = scale * (code + offset),   evaluated in fp64 and rounded once to fp32.
+ * (offset-binary 2-bit data with levels -1.5, -0.5, 0.5, 1.5 times a step: is_signed = 0, offset = -1.5, scale = step.)
+ */
+typedef struct {
+    int32_t bits;      /* 1, 2, 4, 8 or 16 */
+    int32_t is_signed; /* 0: unsigned field, else two's complement */
+    double scale;
+    double offset;
+} pt_quant;
+
+/*
+ * pt_fit_blocks_q -- pt_fit_blocks on quantised samples: every block's row is unpacked to fp32 while it is staged into
+ * shared memory (or, for blocks larger than shared memory, into the workspace row), once per block; everything after
+ * that is pt_fit_blocks, and the results are bit-identical to pt_fit_blocks on the unpacked samples.
+ * xq         [B][row_bytes]  device, packed samples; row_bytes * 8 >= N * bits
+ * quant      [host]
+ * Workspace: pt_fit_blocks_workspace_bytes(B, N, cfg).
+ */
+PT_API int32_t pt_fit_blocks_q(const void* xq, const pt_quant* quant /*[host]*/, int64_t row_bytes, int64_t B, int32_t N,
+                        double fs, const double* lo, const double* hi, const uint32_t* block_index,
+                        const pt_de_config* cfg /*[host]*/, double* best, float* best_rss, uint32_t* status,
+                        float* final_pop, float* final_fit, void* workspace, size_t workspace_bytes, void* stream);
+
+/* pt_unpack_samples -- the same unpacking as a stand-alone call (parity / inspection): xq[B][row_bytes] -> x[B][N] fp32,
+ * both device pointers. */
+PT_API int32_t pt_unpack_samples(const void* xq, const pt_quant* quant /*[host]*/, int64_t row_bytes, int64_t B, int32_t N,
+                          float* x, void* stream);
+
+/*
  * pt_doppler_products -- observables from the fitted parameters, fp64 throughout.  T = N/fs.
  *     phi(t) = phi0 + 2 pi (f t + fdot t^2/2 + fddot t^3/6),  F(t) = dphi/dt  [rad/s]    PAPER.md:228-234 (Eq. 7)
  *     border values at t = -T/2, +T/2, phases reduced to [0, 2 pi)                      PAPER.md:237-246 (Eq. 8)
@@ -168,6 +202,13 @@ PT_API int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, co
                       const pt_de_config* cfg, double los_scale, const int32_t* blocks_per_interval,
                       int32_t n_intervals, double* best, float* best_rss, uint32_t* status, double* per_block,
                       double* total_phase, double* const* interval_out);
+
+/* pt_track_host_q -- pt_track_host on quantised HOST samples xq[B][row_bytes] (see pt_quant): the host-to-device copy
+ * moves the packed bytes (bits/32 of the fp32 volume). */
+PT_API int32_t pt_track_host_q(const void* xq, const pt_quant* quant, int64_t row_bytes, int64_t B, int32_t N, double fs,
+                        const double* lo, const double* hi, const pt_de_config* cfg, double los_scale,
+                        const int32_t* blocks_per_interval, int32_t n_intervals, double* best, float* best_rss,
+                        uint32_t* status, double* per_block, double* total_phase, double* const* interval_out);
 
 /*
  * pt_de_draws -- debug/parity entry: the integer random draws the DE kernel uses, for Q queries.

@@ -25,4 +25,5 @@ from .pt_oracle import (  # noqa: F401
     num_threads,
     philox4x32_10,
     rss,
+    unpack_samples,
 )

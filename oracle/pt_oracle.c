@@ -434,6 +434,39 @@ int32_t pto_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const do
 }
 
 /* ---------------------------------------------------------------------------------------------
+ * Quantised samples.  PAPER.md:104-117 (Table 3): the receiver records 8- or 16-bit (narrow band) and 1-, 2-, 4-
+ * or 8-bit (wide band) samples; "s_i is the quantized signal value".  The paper gives no packing or
+ * level table.  Reading R23: sample n of a block is the bits-wide field n of the block's row, fields
+ * packed from the least significant bit of each byte upwards, 16-bit samples little-endian; the field is read as
+ * an unsigned integer (is_signed = 0) or as two's complement (is_signed = 1); the sample value is
+ *     s_i = scale * (code + offset)
+ * evaluated in fp64 and rounded once to fp32 (the input type of every other function here).
+ * xq[B][row_bytes] -> x[B][N].  Returns -1 on invalid arguments.
+ * ------------------------------------------------------------------------------------------- */
+int32_t pto_unpack_samples(const uint8_t* xq, int64_t row_bytes, int64_t B, int32_t N, int32_t bits, int32_t is_signed,
+                           double scale, double offset, float* x) {
+    if (!xq || !x || B < 1 || N < 1) return -1;
+    if (bits != 1 && bits != 2 && bits != 4 && bits != 8 && bits != 16) return -1;
+    if (row_bytes * 8 < (int64_t)N * bits) return -1;
+    for (int64_t b = 0; b < B; ++b) {
+        const uint8_t* row = xq + b * row_bytes;
+        for (int32_t n = 0; n < N; ++n) {
+            uint32_t field;
+            if (bits == 16) {
+                field = (uint32_t)row[2 * (int64_t)n] | ((uint32_t)row[2 * (int64_t)n + 1] << 8);
+            } else {
+                int64_t bit = (int64_t)n * bits;
+                field = ((uint32_t)row[bit / 8] >> (bit % 8)) & ((1u << bits) - 1u);
+            }
+            int32_t code = (int32_t)field;
+            if (is_signed && (field >> (bits - 1)) & 1u) code = (int32_t)field - (int32_t)(1u << bits);
+            x[b * (int64_t)N + n] = (float)(scale * ((double)code + offset));
+        }
+    }
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------------------------
  * Doppler products.  SURVEY 8(c) item 7.
  *   phi(t) = phi0 + 2 pi (f t + fdot t^2/2 + fddot t^3/6)                  PAPER.md:230 (Eq. 7)
  *   F(t)   = dphi/dt = 2 pi (f + fdot t + fddot t^2/2)   [rad/s]           PAPER.md:232-234 (Eq. 7)

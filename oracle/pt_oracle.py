@@ -74,6 +74,8 @@ def _load():
     lib.pto_de_trial.argtypes = [C.POINTER(_DEConfig), C.c_uint32, C.c_uint32, C.c_uint32, p, C.c_int32, p, p, p]
     lib.pto_fit_blocks.argtypes = [p, C.c_int64, C.c_int32, C.c_double, p, p, C.POINTER(_DEConfig), p, p, p, p, p, p, p]
     lib.pto_fit_blocks.restype = C.c_int32
+    lib.pto_unpack_samples.argtypes = [p, C.c_int64, C.c_int64, C.c_int32, C.c_int32, C.c_int32, C.c_double, C.c_double, p]
+    lib.pto_unpack_samples.restype = C.c_int32
     lib.pto_doppler_products.argtypes = [p, C.c_int64, C.c_int32, C.c_double, C.c_double, p, C.c_int32, p, p, p]
     lib.pto_doppler_products.restype = C.c_int32
     _lib = lib
@@ -220,6 +222,18 @@ def fit_blocks(x, fs: float, lo, hi, *, NP: int, generations: int, F: float = 0.
     if want_trace:
         out["trace"] = trace
     return out
+
+
+def unpack_samples(xq, N: int, bits: int, is_signed: bool, scale: float, offset: float):
+    """xq[B][row_bytes] uint8 -> x[B][N] fp32, s = scale (code + offset) (Table 3 sample formats; reading R23)."""
+    xq = np.ascontiguousarray(xq, dtype=np.uint8)
+    B, row_bytes = xq.shape
+    x = np.zeros((B, int(N)), dtype=np.float32)
+    rc = _load().pto_unpack_samples(_ptr(xq), row_bytes, B, int(N), int(bits), int(bool(is_signed)), float(scale),
+                                    float(offset), _ptr(x))
+    if rc != 0:
+        raise ValueError("pto_unpack_samples: invalid argument")
+    return x
 
 
 def doppler_products(best, T: float, los_scale: float = 0.0, blocks_per_interval=()):

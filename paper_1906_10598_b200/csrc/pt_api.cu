@@ -4,6 +4,7 @@
 #include <cstring>
 #include <cstdlib>
 #include <cmath>
+#include <algorithm>
 #include <vector>
 
 #include "../../include/pt.h"
@@ -288,6 +289,18 @@ static int check_common(long long B, int N, double fs, int NP, int D) {
     return PT_OK;
 }
 
+static int check_quant(const pt_quant* q, int64_t row_bytes, int N, Quant* out) {
+    if (!q) { set_error("quant is null"); return PT_ERR_INVALID_ARG; }
+    if (q->bits != 1 && q->bits != 2 && q->bits != 4 && q->bits != 8 && q->bits != 16) {
+        set_error("quant.bits must be 1, 2, 4, 8 or 16 (got %d)", q->bits);
+        return PT_ERR_INVALID_ARG;
+    }
+    if (!std::isfinite(q->scale) || !std::isfinite(q->offset)) { set_error("quant.scale and quant.offset must be finite"); return PT_ERR_INVALID_ARG; }
+    if (row_bytes * 8 < (int64_t)N * q->bits) { set_error("row_bytes = %lld holds fewer than N = %d samples of %d bits", (long long)row_bytes, N, q->bits); return PT_ERR_INVALID_ARG; }
+    out->bits = q->bits; out->is_signed = q->is_signed ? 1 : 0; out->scale = q->scale; out->offset = q->offset;
+    return PT_OK;
+}
+
 static int check_cfg(const pt_de_config* cfg) {
     if (!cfg) { set_error("cfg is null"); return PT_ERR_INVALID_ARG; }
     if (cfg->generations < 0) { set_error("generations must be >= 0"); return PT_ERR_INVALID_ARG; }
@@ -326,6 +339,15 @@ __global__ void init_population_kernel(const double* __restrict__ lo, const doub
     init_member<D>((uint32_t)i, block_index ? block_index[b] : (uint32_t)b, k0, k1, l, h, th);
 #pragma unroll
     for (int j = 0; j < D; ++j) pop0[k * D + j] = th[j];
+}
+
+__global__ void unpack_samples_kernel(const unsigned char* __restrict__ xq, long long row_bytes, long long B, int N, Quant q,
+                                      float* __restrict__ x) {
+    const long long total = B * (long long)N;
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < total; k += (long long)gridDim.x * blockDim.x) {
+        const long long b = k / N;
+        x[k] = unpack_sample(xq + b * row_bytes, k - b * N, q);
+    }
 }
 
 __global__ void check_box_kernel(const double* __restrict__ lo, const double* __restrict__ hi, long long n, int* bad) {
@@ -400,21 +422,26 @@ int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg, int32_
     return PT_OK;
 }
 
-int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const double* lo, const double* hi,
-                      const uint32_t* block_index, const pt_de_config* cfg, double* best, float* best_rss,
-                      uint32_t* status, float* final_pop, float* final_fit, void* workspace, size_t workspace_bytes,
-                      void* stream) {
-    if (!x || !lo || !hi || !best || !best_rss || !status) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+static int32_t fit_blocks_impl(const float* x, const unsigned char* xq, const pt_quant* quant, int64_t row_bytes, int64_t B,
+                               int32_t N, double fs, const double* lo, const double* hi, const uint32_t* block_index,
+                               const pt_de_config* cfg, double* best, float* best_rss, uint32_t* status, float* final_pop,
+                               float* final_fit, void* workspace, size_t workspace_bytes, void* stream) {
+    if ((!x && !xq) || !lo || !hi || !best || !best_rss || !status) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
     int rc = check_cfg(cfg);
     if (rc) return rc;
     rc = check_common(B, N, fs, cfg->NP, cfg->D);
     if (rc) return rc;
+    BlockParams p;
+    memset(&p, 0, sizeof(p));
+    if (xq) {
+        rc = check_quant(quant, row_bytes, N, &p.q);
+        if (rc) return rc;
+    }
     Plan pl;
     rc = plan_for(B, N, cfg->NP, cfg->D, &pl, true);
     if (rc) return rc;
-    BlockParams p;
-    memset(&p, 0, sizeof(p));
-    p.x = x; p.lo = lo; p.hi = hi; p.block_index = block_index;
+    p.x = x; p.xq = xq; p.row_bytes = row_bytes;
+    p.lo = lo; p.hi = hi; p.block_index = block_index;
     p.best = best; p.best_rss = best_rss; p.status = status; p.final_pop = final_pop; p.final_fit = final_fit;
     p.B = B; p.N = N; p.Npad = pl.Npad; p.NP = cfg->NP; p.NPpad = pl.NPpad; p.G = cfg->generations;
     p.fs = fs; p.t0 = cfg->t0; p.F = cfg->F;
@@ -422,7 +449,7 @@ int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const dou
     p.key0 = (uint32_t)(cfg->seed & 0xFFFFFFFFull); p.key1 = (uint32_t)(cfg->seed >> 32);
     p.Wg = pl.Wg; p.Ws = pl.Ws;
     p.strategy = cfg->strategy == 0 ? kRand1 : cfg->strategy;
-    p.use_bulk = ((N % 4) == 0 && (reinterpret_cast<uintptr_t>(x) % 16) == 0) ? 1 : 0;
+    p.use_bulk = (!xq && (N % 4) == 0 && (reinterpret_cast<uintptr_t>(x) % 16) == 0) ? 1 : 0;
     rc = attach_workspace(&p, pl, workspace, workspace_bytes);
     if (rc) return rc;
     Plan tl;
@@ -438,6 +465,39 @@ int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const dou
     rc = attach_workspace(&q, tl, nullptr, 0);
     if (rc) return rc;
     return dispatch<kModeFit>(q, tl, cfg->D, cfg->objective, (cudaStream_t)stream);
+}
+
+int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const double* lo, const double* hi,
+                      const uint32_t* block_index, const pt_de_config* cfg, double* best, float* best_rss,
+                      uint32_t* status, float* final_pop, float* final_fit, void* workspace, size_t workspace_bytes,
+                      void* stream) {
+    if (!x) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    return fit_blocks_impl(x, nullptr, nullptr, 0, B, N, fs, lo, hi, block_index, cfg, best, best_rss, status, final_pop,
+                           final_fit, workspace, workspace_bytes, stream);
+}
+
+int32_t pt_fit_blocks_q(const void* xq, const pt_quant* quant, int64_t row_bytes, int64_t B, int32_t N, double fs,
+                        const double* lo, const double* hi, const uint32_t* block_index, const pt_de_config* cfg,
+                        double* best, float* best_rss, uint32_t* status, float* final_pop, float* final_fit,
+                        void* workspace, size_t workspace_bytes, void* stream) {
+    if (!xq) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    return fit_blocks_impl(nullptr, static_cast<const unsigned char*>(xq), quant, row_bytes, B, N, fs, lo, hi, block_index,
+                           cfg, best, best_rss, status, final_pop, final_fit, workspace, workspace_bytes, stream);
+}
+
+int32_t pt_unpack_samples(const void* xq, const pt_quant* quant, int64_t row_bytes, int64_t B, int32_t N, float* x,
+                          void* stream) {
+    if (!xq || !x) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    if (B < 1 || N < 1) { set_error("B and N must be >= 1"); return PT_ERR_INVALID_ARG; }
+    Quant q;
+    int rc = check_quant(quant, row_bytes, N, &q);
+    if (rc) return rc;
+    const long long total = B * (long long)N;
+    const int thr = 256;
+    const unsigned grid = (unsigned)std::min<long long>((total + thr - 1) / thr, 148LL * 16);
+    unpack_samples_kernel<<<grid, thr, 0, (cudaStream_t)stream>>>(static_cast<const unsigned char*>(xq), row_bytes, B, N, q, x);
+    if (check_cuda(cudaGetLastError(), "unpack_samples_kernel launch")) return PT_ERR_CUDA;
+    return PT_OK;
 }
 
 int32_t pt_doppler_products(const double* best, int64_t B, int32_t D, double T, double los_scale,
@@ -487,11 +547,16 @@ int32_t pt_peak_probe(int32_t kind, double* ops_per_s) {
     return peak_probe(kind, ops_per_s);
 }
 
-int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, const double* lo, const double* hi,
-                      const pt_de_config* cfg, double los_scale, const int32_t* blocks_per_interval, int32_t n_intervals,
-                      double* best, float* best_rss, uint32_t* status, double* per_block, double* total_phase,
-                      double* const* interval_out) {
-    if (!x || !lo || !hi) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+static int32_t track_host_impl(const float* x, const void* xq, const pt_quant* quant, int64_t row_bytes, int64_t B, int32_t N,
+                               double fs, const double* lo, const double* hi, const pt_de_config* cfg, double los_scale,
+                               const int32_t* blocks_per_interval, int32_t n_intervals, double* best, float* best_rss,
+                               uint32_t* status, double* per_block, double* total_phase, double* const* interval_out) {
+    if ((!x && !xq) || !lo || !hi) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    if (xq) {
+        Quant qq;
+        const int rq = check_quant(quant, row_bytes, N, &qq);
+        if (rq) return rq;
+    }
     int rc = check_cfg(cfg);
     if (rc) return rc;
     rc = check_common(B, N, fs, cfg->NP, cfg->D);
@@ -500,7 +565,7 @@ int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, const dou
     for (long long k = 0; k < B * cfg->D; ++k)
         if (!(lo[k] <= hi[k])) { set_error("lo > hi at element %lld", k); return PT_ERR_INVALID_ARG; }
     const int D = cfg->D;
-    const size_t nx = (size_t)B * N * sizeof(float), nbox = (size_t)B * D * sizeof(double);
+    const size_t nx = xq ? (size_t)B * (size_t)row_bytes : (size_t)B * N * sizeof(float), nbox = (size_t)B * D * sizeof(double);
     // one device arena for everything
     size_t off = 0;
     auto take = [&off](size_t bytes) { size_t o = off; off += (bytes + 255) / 256 * 256; return o; };
@@ -523,13 +588,14 @@ int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, const dou
     std::vector<double*> d_iv(n_intervals > 0 ? n_intervals : 1, nullptr);
     for (int k = 0; k < n_intervals; ++k) d_iv[k] = reinterpret_cast<double*>(arena + o_iv[k]);
     do {
-        if (check_cuda(cudaMemcpyAsync(arena + o_x, x, nx, cudaMemcpyHostToDevice, st), "H2D x")) { ret = PT_ERR_CUDA; break; }
+        if (check_cuda(cudaMemcpyAsync(arena + o_x, xq ? xq : static_cast<const void*>(x), nx, cudaMemcpyHostToDevice, st), "H2D x")) { ret = PT_ERR_CUDA; break; }
         if (check_cuda(cudaMemcpyAsync(arena + o_lo, lo, nbox, cudaMemcpyHostToDevice, st), "H2D lo")) { ret = PT_ERR_CUDA; break; }
         if (check_cuda(cudaMemcpyAsync(arena + o_hi, hi, nbox, cudaMemcpyHostToDevice, st), "H2D hi")) { ret = PT_ERR_CUDA; break; }
-        ret = pt_fit_blocks(reinterpret_cast<float*>(arena + o_x), B, N, fs, reinterpret_cast<double*>(arena + o_lo),
-                            reinterpret_cast<double*>(arena + o_hi), nullptr, cfg, reinterpret_cast<double*>(arena + o_best),
-                            reinterpret_cast<float*>(arena + o_rss), reinterpret_cast<uint32_t*>(arena + o_st), nullptr,
-                            nullptr, ws_bytes ? arena + o_ws : nullptr, ws_bytes, st);
+        ret = fit_blocks_impl(xq ? nullptr : reinterpret_cast<float*>(arena + o_x), xq ? arena + o_x : nullptr, quant, row_bytes, B,
+                              N, fs, reinterpret_cast<double*>(arena + o_lo), reinterpret_cast<double*>(arena + o_hi), nullptr,
+                              cfg, reinterpret_cast<double*>(arena + o_best), reinterpret_cast<float*>(arena + o_rss),
+                              reinterpret_cast<uint32_t*>(arena + o_st), nullptr, nullptr, ws_bytes ? arena + o_ws : nullptr,
+                              ws_bytes, st);
         if (ret) break;
         ret = pt_doppler_products(reinterpret_cast<double*>(arena + o_best), B, D, (double)N / fs, los_scale,
                                   blocks_per_interval, n_intervals, reinterpret_cast<double*>(arena + o_pb),
@@ -551,6 +617,24 @@ int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, const dou
     cudaStreamDestroy(st);
     cudaFree(arena);
     return ret;
+}
+
+int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, const double* lo, const double* hi,
+                      const pt_de_config* cfg, double los_scale, const int32_t* blocks_per_interval, int32_t n_intervals,
+                      double* best, float* best_rss, uint32_t* status, double* per_block, double* total_phase,
+                      double* const* interval_out) {
+    if (!x) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    return track_host_impl(x, nullptr, nullptr, 0, B, N, fs, lo, hi, cfg, los_scale, blocks_per_interval, n_intervals, best,
+                           best_rss, status, per_block, total_phase, interval_out);
+}
+
+int32_t pt_track_host_q(const void* xq, const pt_quant* quant, int64_t row_bytes, int64_t B, int32_t N, double fs,
+                        const double* lo, const double* hi, const pt_de_config* cfg, double los_scale,
+                        const int32_t* blocks_per_interval, int32_t n_intervals, double* best, float* best_rss,
+                        uint32_t* status, double* per_block, double* total_phase, double* const* interval_out) {
+    if (!xq) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    return track_host_impl(nullptr, xq, quant, row_bytes, B, N, fs, lo, hi, cfg, los_scale, blocks_per_interval, n_intervals,
+                           best, best_rss, status, per_block, total_phase, interval_out);
 }
 
 }  // extern "C"

@@ -36,7 +36,10 @@ enum Mode { kModeFit = 0, kModeFitness = 1 };
 enum Objective { kObjChi2 = 0, kObjCor = 1 };
 
 struct BlockParams {
-    const float* x;               // [B][N]
+    const float* x;               // [B][N] fp32 samples, or null when the samples are quantised:
+    const unsigned char* xq;      // [B][row_bytes] packed samples (Quant q says how), unpacked while staging
+    long long row_bytes;
+    Quant q;
     const double* lo;             // [B][D]  (fit)
     const double* hi;             // [B][D]  (fit)
     const uint32_t* block_index;  // [B] or null (fit)
@@ -457,17 +460,23 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
     };
 
     for (long long blk = p.blk0 + first_blk; blk < p.B; blk += blk_stride) {
-        const float* xg = p.x + blk * (long long)p.N + n_lo;      // this CTA's slice of the block
+        const bool quantised = p.q.bits != 0;
+        const float* xg = quantised ? nullptr : p.x + blk * (long long)p.N + n_lo;      // this CTA's slice of the block
+        const unsigned char* xqrow = quantised ? p.xq + blk * p.row_bytes : nullptr;
         // ---- a0: stage the block's samples (PAPER.md:121 data block) into shared memory, once ----
-        //      (streamed path: tiles are staged every pass; an unaligned row is first copied to the workspace)
+        //      (streamed path: tiles are staged every pass; an unaligned or quantised row is first written to the
+        //       workspace as fp32).  Quantised samples (Table 3) are unpacked here, once per block.
         float* wrow = STREAM ? p.ws_wref + (size_t)blockIdx.x * p.Npad : nullptr;
         const float* xrow = xg;
         if (STREAM) {
-            if (!p.use_bulk) {
+            if (quantised || !p.use_bulk) {
                 float* xw = p.ws_x + (size_t)blockIdx.x * p.Npad;
-                for (int n = tid; n < p.Npad; n += nthr) xw[n] = (n < p.N) ? __ldg(xg + n) : 0.0f;
+                if (quantised) for (int n = tid; n < p.Npad; n += nthr) xw[n] = (n < p.N) ? unpack_sample(xqrow, n, p.q) : 0.0f;
+                else for (int n = tid; n < p.Npad; n += nthr) xw[n] = (n < p.N) ? __ldg(xg + n) : 0.0f;
                 xrow = xw;
             }
+        } else if (quantised) {
+            for (int n = tid; n < sl.N; n += nthr) xs[n] = unpack_sample(xqrow, (long long)n_lo + n, p.q);
         } else if (p.use_bulk) {
             if (tid == 0) {
                 fence_proxy_async();   // earlier generic-proxy reads of xs are ordered before the async writes

@@ -170,6 +170,30 @@ __device__ __forceinline__ double mutant_coord(int strategy, double xi, double x
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Quantised samples (Table 3: 1/2/4/8/16-bit recording modes; reading R23).
+// Sample n of a row is its bits-wide field n, packed from the least significant bit of each byte upwards (16-bit:
+// little-endian); read as unsigned or two's complement; value = scale (code + offset) in fp64, rounded once to fp32.
+// ---------------------------------------------------------------------------------------------------
+struct Quant {
+    int bits;          // 0: the samples are fp32 already
+    int is_signed;
+    double scale, offset;
+};
+
+__device__ __forceinline__ float unpack_sample(const unsigned char* __restrict__ row, long long n, const Quant& q) {
+    uint32_t field;
+    if (q.bits == 16) {
+        field = (uint32_t)__ldg(row + 2 * n) | ((uint32_t)__ldg(row + 2 * n + 1) << 8);
+    } else {
+        const long long bit = n * q.bits;
+        field = ((uint32_t)__ldg(row + (bit >> 3)) >> (int)(bit & 7)) & ((1u << q.bits) - 1u);
+    }
+    int code = (int)field;
+    if (q.is_signed && ((field >> (q.bits - 1)) & 1u)) code = (int)field - (int)(1u << q.bits);
+    return __double2float_rn(__dmul_rn(q.scale, __dadd_rn((double)code, q.offset)));
+}
+
+// ---------------------------------------------------------------------------------------------------
 // mbarrier + 1-D bulk async copy (TMA engine, SASS UBLKCP) -- global -> shared staging of a data block.
 // ---------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }

@@ -37,6 +37,12 @@ class DEConfig(C.Structure):
     ]
 
 
+class Quant(C.Structure):
+    """Mirror of ``pt_quant`` (include/pt.h): s = scale * (code + offset)."""
+
+    _fields_ = [("bits", C.c_int32), ("is_signed", C.c_int32), ("scale", C.c_double), ("offset", C.c_double)]
+
+
 def lib():
     """Load (building first if needed) the CUDA library.  Raises if that is impossible."""
     global _lib
@@ -59,6 +65,12 @@ def lib():
     L.pt_fit_blocks_workspace_bytes.restype = sz
     L.pt_fit_blocks.argtypes = [p, i64, i32, f64, p, p, p, C.POINTER(DEConfig), p, p, p, p, p, p, sz, p]
     L.pt_fit_blocks.restype = i32
+    L.pt_fit_blocks_q.argtypes = [p, C.POINTER(Quant), i64, i64, i32, f64, p, p, p, C.POINTER(DEConfig), p, p, p, p, p, p, sz, p]
+    L.pt_fit_blocks_q.restype = i32
+    L.pt_unpack_samples.argtypes = [p, C.POINTER(Quant), i64, i64, i32, p, p]
+    L.pt_unpack_samples.restype = i32
+    L.pt_track_host_q.argtypes = [p, C.POINTER(Quant), i64, i64, i32, f64, p, p, C.POINTER(DEConfig), f64, p, i32, p, p, p, p, p, p]
+    L.pt_track_host_q.restype = i32
     L.pt_fit_blocks_plan.argtypes = [i64, i32, C.POINTER(DEConfig), p]
     L.pt_fit_blocks_plan.restype = i32
     L.pt_doppler_products.argtypes = [p, i64, i32, f64, f64, p, i32, p, p, p, p]
@@ -139,11 +151,30 @@ def pt_objective(x: torch.Tensor, fs: float, pop: torch.Tensor, objective: int, 
     return out
 
 
+def make_quant(bits: int, is_signed: bool, scale: float, offset: float = 0.0) -> Quant:
+    return Quant(int(bits), int(bool(is_signed)), float(scale), float(offset))
+
+
+def pt_unpack_samples(xq: torch.Tensor, N: int, quant: Quant) -> torch.Tensor:
+    """xq[B][row_bytes] uint8 (device) -> x[B][N] fp32."""
+    B, row_bytes = xq.shape
+    x = torch.empty((B, int(N)), dtype=torch.float32, device=xq.device)
+    rc = lib().pt_unpack_samples(_dev(xq, torch.uint8, "xq"), C.byref(quant), row_bytes, B, int(N), x.data_ptr(), _stream())
+    _check(rc, "pt_unpack_samples")
+    return x
+
+
 def pt_fit_blocks(x: torch.Tensor, fs: float, lo: torch.Tensor, hi: torch.Tensor, cfg: DEConfig, *,
-                  block_index: torch.Tensor | None = None, want_pop: bool = False) -> dict:
+                  block_index: torch.Tensor | None = None, want_pop: bool = False, quant: Quant | None = None,
+                  N: int | None = None) -> dict:
     """DE fit of every block; returns dict(best[B][D] f64, best_rss[B] f32, status[B] i32-view of u32
-    [, final_pop[B][NP][D] f32, final_fit[B][NP] f32])."""
-    B, N = x.shape
+    [, final_pop[B][NP][D] f32, final_fit[B][NP] f32]).  With ``quant`` x is uint8 [B][row_bytes] of packed samples
+    (pt_fit_blocks_q) and ``N`` is the number of samples per block."""
+    if quant is None:
+        B, N = x.shape
+    else:
+        B, row_bytes = x.shape
+        N = int(N)
     D, NP = cfg.D, cfg.NP
     if tuple(lo.shape) != (B, D) or tuple(hi.shape) != (B, D):
         raise PtError("lo and hi must be [B][D]")
@@ -156,11 +187,13 @@ def pt_fit_blocks(x: torch.Tensor, fs: float, lo: torch.Tensor, hi: torch.Tensor
     ws_bytes = lib().pt_fit_blocks_workspace_bytes(B, N, C.byref(cfg))
     ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev) if ws_bytes else None
     bidx = None if block_index is None else _dev(block_index, torch.int32, "block_index")
-    rc = lib().pt_fit_blocks(_dev(x, torch.float32, "x"), B, N, float(fs), _dev(lo, torch.float64, "lo"),
-                             _dev(hi, torch.float64, "hi"), bidx, C.byref(cfg), best.data_ptr(), best_rss.data_ptr(),
-                             status.data_ptr(), fpop.data_ptr() if want_pop else None,
-                             ffit.data_ptr() if want_pop else None, ws.data_ptr() if ws is not None else None, ws_bytes,
-                             _stream())
+    tail = (_dev(lo, torch.float64, "lo"), _dev(hi, torch.float64, "hi"), bidx, C.byref(cfg), best.data_ptr(),
+            best_rss.data_ptr(), status.data_ptr(), fpop.data_ptr() if want_pop else None,
+            ffit.data_ptr() if want_pop else None, ws.data_ptr() if ws is not None else None, ws_bytes, _stream())
+    if quant is None:
+        rc = lib().pt_fit_blocks(_dev(x, torch.float32, "x"), B, N, float(fs), *tail)
+    else:
+        rc = lib().pt_fit_blocks_q(_dev(x, torch.uint8, "xq"), C.byref(quant), row_bytes, B, N, float(fs), *tail)
     _check(rc, "pt_fit_blocks")
     out = {"best": best, "best_rss": best_rss, "status": status}
     if want_pop:
@@ -192,11 +225,17 @@ def pt_doppler_products(best: torch.Tensor, T: float, los_scale: float = 0.0, bl
     return per_block, total, outs
 
 
-def pt_track_host(x, fs: float, lo, hi, cfg: DEConfig, los_scale: float = 0.0, blocks_per_interval=()):
-    """Whole hot path on HOST tensors (CPU torch tensors, ideally pinned): H2D, fit, products, D2H."""
-    B, N = x.shape
+def pt_track_host(x, fs: float, lo, hi, cfg: DEConfig, los_scale: float = 0.0, blocks_per_interval=(),
+                  quant: Quant | None = None, N: int | None = None):
+    """Whole hot path on HOST tensors (CPU torch tensors, ideally pinned): H2D, fit, products, D2H.  With ``quant``
+    x is uint8 [B][row_bytes] of packed samples (pt_track_host_q) and ``N`` the samples per block."""
+    if quant is None:
+        B, N = x.shape
+    else:
+        B, row_bytes = x.shape
+        N = int(N)
     D = cfg.D
-    for t, dt, nm in ((x, torch.float32, "x"), (lo, torch.float64, "lo"), (hi, torch.float64, "hi")):
+    for t, dt, nm in ((x, torch.float32 if quant is None else torch.uint8, "x"), (lo, torch.float64, "lo"), (hi, torch.float64, "hi")):
         if t.is_cuda or t.dtype != dt or not t.is_contiguous():
             raise PtError("%s must be a contiguous host tensor of dtype %s" % (nm, dt))
     m = [int(v) for v in blocks_per_interval]
@@ -208,9 +247,12 @@ def pt_track_host(x, fs: float, lo, hi, cfg: DEConfig, los_scale: float = 0.0, b
     outs = [torch.empty((B // v, 2), dtype=torch.float64) for v in m]
     m_arr = (C.c_int32 * max(len(m), 1))(*m)
     ptrs = (C.c_void_p * max(len(m), 1))(*[o.data_ptr() if o.numel() else None for o in outs])
-    rc = lib().pt_track_host(x.data_ptr(), B, N, float(fs), lo.data_ptr(), hi.data_ptr(), C.byref(cfg), float(los_scale),
-                             m_arr, len(m), best.data_ptr(), best_rss.data_ptr(), status.data_ptr(), per_block.data_ptr(),
-                             total.data_ptr(), ptrs)
+    tail = (B, N, float(fs), lo.data_ptr(), hi.data_ptr(), C.byref(cfg), float(los_scale), m_arr, len(m), best.data_ptr(),
+            best_rss.data_ptr(), status.data_ptr(), per_block.data_ptr(), total.data_ptr(), ptrs)
+    if quant is None:
+        rc = lib().pt_track_host(x.data_ptr(), *tail)
+    else:
+        rc = lib().pt_track_host_q(x.data_ptr(), C.byref(quant), row_bytes, *tail)
     _check(rc, "pt_track_host")
     return {"best": best, "best_rss": best_rss, "status": status, "per_block": per_block, "total_phase": total,
             "intervals": outs}

@@ -308,3 +308,45 @@ def oracle_subset(config: int) -> list[int]:
     if config == 3:
         return sorted(set(range(60)) | set(range(0, 36000, 1000)))
     raise ValueError("subset is defined for configs 2 and 3")
+
+
+# ------------------------------------------------------------------------------------------
+# Quantised recordings (Table 3: 8/16-bit narrow-band and 1/2/4/8-bit wide-band modes).
+# This is the receiver's A/D converter, i.e. input synthesis; unpacking belongs to the method (oracle / CUDA path).
+# ------------------------------------------------------------------------------------------
+def quantise(x: np.ndarray, bits: int):
+    """Quantise fp32 samples x[B][N] to `bits`-wide codes and pack them, fields from the least significant bit of
+    each byte upwards (16-bit: little-endian).  Returns (xq uint8 [B][row_bytes], quant dict) with
+    quant = dict(bits, is_signed, scale, offset) such that the sample value is scale * (code + offset).
+
+    8 and 16 bits: two's complement, full scale = the largest |x| of the array.
+    1, 2, 4 bits: offset binary with L = 2^bits levels at (code - (L-1)/2) * step; step = 2 rms (1 bit: levels
+    +-rms), rms (2 bits: thresholds at 0 and +-rms, close to the optimal 4-level quantiser of Gaussian noise),
+    0.335 rms (4 bits, the optimal 16-level step)."""
+    x = np.asarray(x, dtype=np.float32)
+    B, N = x.shape
+    if bits in (8, 16):
+        full = float(np.max(np.abs(x)))
+        qmax = (1 << (bits - 1)) - 1
+        scale = full / qmax if full > 0 else 1.0
+        code = np.clip(np.rint(x.astype(np.float64) / scale), -qmax - 1, qmax).astype(np.int64)
+        quant = dict(bits=bits, is_signed=True, scale=scale, offset=0.0)
+        if bits == 8:
+            xq = code.astype(np.int8).view(np.uint8)
+        else:
+            xq = code.astype("<i2").view(np.uint8).reshape(B, 2 * N)
+        return np.ascontiguousarray(xq), quant
+    if bits not in (1, 2, 4):
+        raise ValueError("bits must be 1, 2, 4, 8 or 16")
+    if (N * bits) % 8:
+        raise ValueError("N * bits must be a multiple of 8")
+    L = 1 << bits
+    rms = float(np.sqrt(np.mean(x.astype(np.float64) ** 2)))
+    step = {1: 2.0, 2: 1.0, 4: 0.335}[bits] * rms
+    offset = -(L - 1) / 2.0
+    code = np.clip(np.floor(x.astype(np.float64) / step - offset + 0.5), 0, L - 1).astype(np.uint8)
+    per = 8 // bits
+    fields = code.reshape(B, N // per, per).astype(np.uint16)
+    shifts = (np.arange(per) * bits).astype(np.uint16)
+    xq = np.bitwise_or.reduce(fields << shifts, axis=-1).astype(np.uint8)
+    return np.ascontiguousarray(xq), dict(bits=bits, is_signed=False, scale=step, offset=offset)

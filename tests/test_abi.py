@@ -44,11 +44,28 @@ def test_header_compiles_as_plain_c(tmp_path):
                     str(tmp_path / "t.o")], check=True)
 
 
-def test_config_struct_layout_matches_binding():
-    from paper_1906_10598_b200.pt import DEConfig
-    # int32 x3, pad, double x2, uint64, double = 48 bytes with natural alignment
-    assert C.sizeof(DEConfig) == 48
-    assert DEConfig.F.offset == 16 and DEConfig.seed.offset == 32 and DEConfig.t0.offset == 40
+def test_struct_layouts_match_the_binding(tmp_path):
+    """sizeof / offsetof of pt_de_config and pt_quant as gcc lays them out from include/pt.h = the ctypes mirrors."""
+    import subprocess
+    from paper_1906_10598_b200.pt import DEConfig, Quant
+    fields = {"pt_de_config": [f for f, _ in DEConfig._fields_], "pt_quant": [f for f, _ in Quant._fields_]}
+    body = ['#include <stdio.h>', '#include <stddef.h>', '#include "pt.h"', 'int main(void){']
+    for st, names in fields.items():
+        body.append('printf("%%zu", sizeof(%s));' % st)
+        for f in names:
+            body.append('printf(" %%zu", offsetof(%s, %s));' % (st, f))
+        body.append('printf("\\n");')
+    body.append('return 0;}')
+    src = tmp_path / "layout.c"
+    src.write_text("\n".join(body))
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-std=c99", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
+    lines = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.strip().splitlines()
+    for line, (st, names), cls in zip(lines, fields.items(), (DEConfig, Quant)):
+        nums = [int(v) for v in line.split()]
+        assert nums[0] == C.sizeof(cls), st
+        assert nums[1:] == [getattr(cls, f).offset for f in names], st
+    assert C.sizeof(DEConfig) == 56 and DEConfig.strategy.offset == 48 and DEConfig.objective.offset == 52
 
 
 def test_argument_validation_needs_no_gpu(lib_path):
@@ -77,6 +94,18 @@ def test_argument_validation_needs_no_gpu(lib_path):
     assert L.pt_doppler_products(dummy, 0, 5, 1.0, 0.0, None, 0, dummy, dummy, None, None) == -1
     assert L.pt_doppler_products(dummy, 4, 5, -1.0, 0.0, None, 0, dummy, dummy, None, None) == -1
     assert L.pt_version().startswith(b"pt ")
+    # widened rows: objective / strategy / quantised input are validated before any CUDA call
+    assert L.pt_objective(dummy, 1, 1000, 1000.0, -0.5, dummy, 60, 5, 2, dummy, None, 0, None) == -1
+    assert call(cfg=pt.make_config(D=5, NP=60, generations=1, t0=0.0, strategy=7)) == -1
+    assert call(cfg=pt.make_config(D=5, NP=60, generations=1, t0=0.0, objective=3)) == -1
+    q = pt.make_quant(8, True, 1.0)
+    assert L.pt_fit_blocks_q(None, C.byref(q), 1000, 1, 1000, 1000.0, dummy, dummy, None, C.byref(cfg), dummy, dummy, dummy,
+                             None, None, None, 0, None) == -1
+    assert L.pt_fit_blocks_q(dummy, C.byref(pt.make_quant(3, True, 1.0)), 1000, 1, 1000, 1000.0, dummy, dummy, None,
+                             C.byref(cfg), dummy, dummy, dummy, None, None, None, 0, None) == -1
+    assert L.pt_fit_blocks_q(dummy, C.byref(q), 999, 1, 1000, 1000.0, dummy, dummy, None, C.byref(cfg), dummy, dummy, dummy,
+                             None, None, None, 0, None) == -1            # row shorter than N samples
+    assert L.pt_unpack_samples(dummy, C.byref(q), 10, 1, 0, dummy, None) == -1
 
 
 def test_plan_is_computable_without_gpu(lib_path):
