@@ -5,8 +5,10 @@ TEST INFRASTRUCTURE, NOT THE PRODUCT: only ``tests/``, ``__graft_entry__.smoke()
 nothing from ``paper_1906_10598_b200`` and shares no code with the CUDA path.
 
 ``oracle/pt_oracle.c`` holds the arithmetic (plain C, fp64, exact-integer Philox); this package
-only compiles it with gcc and marshals numpy arrays into it with ctypes.
+only compiles it with gcc and marshals numpy arrays into it with ctypes.  ``oracle/pt_acquire.py`` is the
+fp64 numpy statement of the paper's initial range determination (FFT acquisition).
 """
+from .pt_acquire import acquire, piece_estimate  # noqa: F401
 from .pt_oracle import (  # noqa: F401
     aux_uniforms,
     build,
