@@ -172,6 +172,37 @@ PT_API int32_t pt_unpack_samples(const void* xq, const pt_quant* quant /*[host]*
                           float* x, void* stream);
 
 /*
+ * pt_acquire -- initial range determination (section 3.1.1 items 1-6): per block, the centre frequency
+ * and amplitude from the FFT of "a small piece of data extracted from block center", the frequency rate by "central
+ * difference method through three equally spaced frequency values near block center", and the parameter boxes
+ *     phi0 in [-pi, pi] (item 1: a full turn), f in f_c -+ max(f_rel |f_c|, f_bins fs/M) (item 2: +-10 %),
+ *     fdot in fdot_est -+ fdot_bins (fs/M)/(spacing/fs) (the paper gives no range for c2), fddot in -+ fddot_hw
+ *     (item 4: c3 in [-50, 50], i.e. 150/pi), a0 in a_est (1 -+ a_rel) (item 5: +-10 %), a1 in -+ a1_rel a_est/T (item 6).
+ * What the paper leaves open (reading R24): piece k = -1, 0, 1 is samples [N/2 + k spacing - M/2, N/2 + k spacing
+ * + M/2) of the block, weighted by the periodic Hann window; its frequency is the largest |X_k|^2 over 1 <= k <= M/2 - 1
+ * (lowest k on ties) refined by a parabola through the logarithms of the three powers around it; its amplitude is
+ * 4 |X_k| / M divided by the Hann main-lobe factor sinc(delta)/(1 - delta^2).
+ * x    [B][N]  fp32 samples (device)
+ * acq  [host]  M: power of two, 8 <= M <= 8192, M + 2 spacing <= N, spacing >= 1
+ * est  [B][8]  fp64 out: a_est, f(-1), f(0), f(+1), fdot_est, peak bins of the three pieces
+ * lo, hi [B][D] fp64 out: the boxes, ready for pt_fit_blocks
+ * All blocks are independent: one CTA per block, no sequential dependence between blocks.
+ */
+typedef struct {
+    int32_t M;        /* piece length (power of two)                                              */
+    int32_t spacing;  /* samples between piece centres                                            */
+    double f_rel;     /* 0.1 in the paper                                          */
+    double f_bins;    /* alternative half-width in FFT bins (the larger of the two is taken)      */
+    double fdot_bins; /* half-width of fdot in frequency bins per spacing                         */
+    double a_rel;     /* 0.1 in the paper                                          */
+    double a1_rel;    /* 0.2 in the paper                                          */
+    double fddot_hw;  /* 150/pi in the paper's units; used when D = 6              */
+} pt_acq_config;
+
+PT_API int32_t pt_acquire(const float* x, int64_t B, int32_t N, double fs, int32_t D, const pt_acq_config* acq /*[host]*/,
+                   double* est, double* lo, double* hi, void* stream);
+
+/*
  * pt_doppler_products -- observables from the fitted parameters, fp64 throughout.  T = N/fs.
  *     phi(t) = phi0 + 2 pi (f t + fdot t^2/2 + fddot t^3/6),  F(t) = dphi/dt  [rad/s]    PAPER.md:228-234 (Eq. 7)
  *     border values at t = -T/2, +T/2, phases reduced to [0, 2 pi)                      PAPER.md:237-246 (Eq. 8)

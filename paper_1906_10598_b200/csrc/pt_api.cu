@@ -500,6 +500,23 @@ int32_t pt_unpack_samples(const void* xq, const pt_quant* quant, int64_t row_byt
     return PT_OK;
 }
 
+int32_t pt_acquire(const float* x, int64_t B, int32_t N, double fs, int32_t D, const pt_acq_config* acq, double* est,
+                   double* lo, double* hi, void* stream) {
+    if (!x || !acq || !est || !lo || !hi) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    if (B < 1 || N < 8 || !(fs > 0.0) || (D != 5 && D != 6)) { set_error("invalid B, N, fs or D"); return PT_ERR_INVALID_ARG; }
+    const int M = acq->M;
+    if (M < 8 || (M & (M - 1))) { set_error("acq.M must be a power of two >= 8 (got %d)", M); return PT_ERR_INVALID_ARG; }
+    if (M > 8192) { set_error("acq.M = %d exceeds the compiled limit 8192", M); return PT_ERR_UNSUPPORTED; }
+    if (acq->spacing < 1 || (long long)M + 2LL * acq->spacing > N) { set_error("pieces do not fit: M + 2 spacing must be <= N"); return PT_ERR_INVALID_ARG; }
+    const double v[6] = {acq->f_rel, acq->f_bins, acq->fdot_bins, acq->a_rel, acq->a1_rel, acq->fddot_hw};
+    for (int k = 0; k < 6; ++k)
+        if (!(v[k] >= 0.0) || !std::isfinite(v[k])) { set_error("acq half-widths must be finite and >= 0"); return PT_ERR_INVALID_ARG; }
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0) { (void)cudaGetLastError(); set_error("no CUDA device"); return PT_ERR_CUDA; }
+    if (acquire_launch(x, B, N, fs, D, acq, est, lo, hi, (cudaStream_t)stream)) return PT_ERR_CUDA;
+    return PT_OK;
+}
+
 int32_t pt_doppler_products(const double* best, int64_t B, int32_t D, double T, double los_scale,
                             const int32_t* blocks_per_interval, int32_t n_intervals, double* per_block,
                             double* total_phase, double* const* interval_out, void* stream) {

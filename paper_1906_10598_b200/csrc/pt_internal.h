@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "../../include/pt.h"
 #include "pt_device.cuh"
 
 namespace pt {
@@ -10,6 +11,10 @@ namespace pt {
 // pt_doppler.cu
 int doppler_launch(const double* best, long long B, int D, double T, double los_scale, const int32_t* m, int n_intervals,
                    double* per_block, double* total_phase, double* const* interval_out, cudaStream_t st);
+
+// pt_acquire.cu
+int acquire_launch(const float* x, long long B, int N, double fs, int D, const pt_acq_config* a, double* est, double* lo,
+                   double* hi, cudaStream_t st);
 
 // pt_probe.cu
 int peak_probe(int kind, double* ops_per_s);

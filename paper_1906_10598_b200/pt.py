@@ -43,6 +43,13 @@ class Quant(C.Structure):
     _fields_ = [("bits", C.c_int32), ("is_signed", C.c_int32), ("scale", C.c_double), ("offset", C.c_double)]
 
 
+class AcqConfig(C.Structure):
+    """Mirror of ``pt_acq_config`` (include/pt.h)."""
+
+    _fields_ = [("M", C.c_int32), ("spacing", C.c_int32), ("f_rel", C.c_double), ("f_bins", C.c_double),
+                ("fdot_bins", C.c_double), ("a_rel", C.c_double), ("a1_rel", C.c_double), ("fddot_hw", C.c_double)]
+
+
 def lib():
     """Load (building first if needed) the CUDA library.  Raises if that is impossible."""
     global _lib
@@ -71,6 +78,8 @@ def lib():
     L.pt_unpack_samples.restype = i32
     L.pt_track_host_q.argtypes = [p, C.POINTER(Quant), i64, i64, i32, f64, p, p, C.POINTER(DEConfig), f64, p, i32, p, p, p, p, p, p]
     L.pt_track_host_q.restype = i32
+    L.pt_acquire.argtypes = [p, i64, i32, f64, i32, C.POINTER(AcqConfig), p, p, p, p]
+    L.pt_acquire.restype = i32
     L.pt_fit_blocks_plan.argtypes = [i64, i32, C.POINTER(DEConfig), p]
     L.pt_fit_blocks_plan.restype = i32
     L.pt_doppler_products.argtypes = [p, i64, i32, f64, f64, p, i32, p, p, p, p]
@@ -200,6 +209,26 @@ def pt_fit_blocks(x: torch.Tensor, fs: float, lo: torch.Tensor, hi: torch.Tensor
         out["final_pop"] = fpop
         out["final_fit"] = ffit
     return out
+
+
+def make_acq_config(*, M: int, spacing: int, f_rel: float = 0.1, f_bins: float = 0.0, fdot_bins: float = 1.0,
+                    a_rel: float = 0.1, a1_rel: float = 0.2, fddot_hw: float = 47.746482927568600) -> AcqConfig:
+    """Defaults are the paper's percentages; fddot_hw = 150/pi is c3 in [-50, 50]."""
+    return AcqConfig(int(M), int(spacing), float(f_rel), float(f_bins), float(fdot_bins), float(a_rel), float(a1_rel),
+                     float(fddot_hw))
+
+
+def pt_acquire(x: torch.Tensor, fs: float, D: int, acq: AcqConfig) -> dict:
+    """Initial ranges of every block: dict(est[B][8], lo[B][D], hi[B][D]) fp64 on the device."""
+    B, N = x.shape
+    dev = x.device
+    est = torch.empty((B, 8), dtype=torch.float64, device=dev)
+    lo = torch.empty((B, int(D)), dtype=torch.float64, device=dev)
+    hi = torch.empty((B, int(D)), dtype=torch.float64, device=dev)
+    rc = lib().pt_acquire(_dev(x, torch.float32, "x"), B, N, float(fs), int(D), C.byref(acq), est.data_ptr(), lo.data_ptr(),
+                          hi.data_ptr(), _stream())
+    _check(rc, "pt_acquire")
+    return {"est": est, "lo": lo, "hi": hi}
 
 
 def pt_fit_blocks_plan(B: int, N: int, cfg: DEConfig) -> dict:
