@@ -9,6 +9,7 @@ only compiles it with gcc and marshals numpy arrays into it with ctypes.  ``orac
 fp64 numpy statement of the paper's initial range determination (FFT acquisition).
 """
 from .pt_acquire import acquire, piece_estimate  # noqa: F401
+from .pt_retry import doubtful_blocks, extrapolated_box, refit_doubtful  # noqa: F401
 from .pt_oracle import (  # noqa: F401
     aux_uniforms,
     build,
