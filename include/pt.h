@@ -203,6 +203,42 @@ PT_API int32_t pt_acquire(const float* x, int64_t B, int32_t N, double fs, int32
                    double* est, double* lo, double* hi, void* stream);
 
 /*
+ * pt_refit_doubtful -- continuity check and re-search of doubtful blocks (section 3.1.3, Eq. 8: a solution
+ * is judged by "the continuity of instantaneous phase and frequency at the bound of two adjacent data block ... within
+ * the threshold of noise"; :191-197 run-time ranges extrapolated from a solved block; :252 "the software will
+ * automatically adjust parameters range and try to search again.  The data block will be abandoned after three attempts").
+ * The paper walks the blocks one by one; here all blocks are fitted first (pt_fit_blocks) and then, per attempt a = 1 ..
+ * max_attempts (reading R25):
+ *   border j (blocks j, j+1) is bad if |wrapped phase residual| > phi_tol or |frequency residual| > F_tol;
+ *   a block is doubtful if every border it has is bad;
+ *   a doubtful block b takes ranges from the nearest trusted block n (left on equal distance), k = b - n, with
+ *   F(t) = f + fdot t + fddot t^2/2 of block n:  f in mid[F((k-1/2)T), F((k+1/2)T)] -+ g max(half distance, f_floor),
+ *   fdot likewise from F'(t) with fdot_floor, a0 in a0^n (1 -+ g a_rel), phi0 in [-pi, pi], a1 and fddot unchanged,
+ *   g = grow^(a-1); with no trusted block its own box is widened by grow;
+ *   the doubtful blocks (only they) are fitted again with key seed + a * 0x9E3779B97F4A7C15 and replace their solution.
+ * Blocks still doubtful after the last attempt get status bit 2 (value 4, "abandoned").
+ * lo, hi, best, best_rss, status [B]... are those of the preceding pt_fit_blocks call and are updated in place;
+ * attempts [B] int32 device out: re-searches each block took (set to 0 first).
+ * workspace: >= pt_refit_doubtful_workspace_bytes(B, N, cfg) device bytes, 16-byte aligned.
+ * The call synchronises `stream` once per attempt (the list of doubtful blocks is compacted on the host).
+ */
+typedef struct {
+    double phi_tol;       /* rad                                                              */
+    double F_tol;         /* Hz                                                               */
+    int32_t max_attempts; /* 3 in the paper                                    */
+    double grow;          /* enlargement of the ranges per attempt                            */
+    double f_floor;       /* Hz: smallest half-width of the extrapolated f range (times g)    */
+    double fdot_floor;    /* Hz/s                                                             */
+    double a_rel;         /* 0.1 in the paper                                  */
+} pt_retry_config;
+
+PT_API size_t pt_refit_doubtful_workspace_bytes(int64_t B, int32_t N, const pt_de_config* cfg /*[host]*/);
+PT_API int32_t pt_refit_doubtful(const float* x, int64_t B, int32_t N, double fs, double* lo, double* hi,
+                          const uint32_t* block_index, const pt_de_config* cfg /*[host]*/,
+                          const pt_retry_config* retry /*[host]*/, double* best, float* best_rss, uint32_t* status,
+                          int32_t* attempts, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * pt_doppler_products -- observables from the fitted parameters, fp64 throughout.  T = N/fs.
  *     phi(t) = phi0 + 2 pi (f t + fdot t^2/2 + fddot t^3/6),  F(t) = dphi/dt  [rad/s]    PAPER.md:228-234 (Eq. 7)
  *     border values at t = -T/2, +T/2, phases reduced to [0, 2 pi)                      PAPER.md:237-246 (Eq. 8)

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpt.so")
 STAMP = os.path.join(HERE, ".libpt.stamp")
-SOURCES = ["pt_api.cu", "pt_doppler.cu", "pt_probe.cu", "pt_acquire.cu"]
+SOURCES = ["pt_api.cu", "pt_doppler.cu", "pt_probe.cu", "pt_acquire.cu", "pt_retry.cu"]
 NVCC_FLAGS = [
     "-O3",
     "-std=c++17",

@@ -425,7 +425,9 @@ int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg, int32_
 static int32_t fit_blocks_impl(const float* x, const unsigned char* xq, const pt_quant* quant, int64_t row_bytes, int64_t B,
                                int32_t N, double fs, const double* lo, const double* hi, const uint32_t* block_index,
                                const pt_de_config* cfg, double* best, float* best_rss, uint32_t* status, float* final_pop,
-                               float* final_fit, void* workspace, size_t workspace_bytes, void* stream) {
+                               float* final_fit, void* workspace, size_t workspace_bytes, void* stream,
+                               const uint32_t* sel = nullptr) {
+    // sel != null: B work items, item j is data block sel[j] of the caller's arrays (pt_refit_doubtful)
     if ((!x && !xq) || !lo || !hi || !best || !best_rss || !status) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
     int rc = check_cfg(cfg);
     if (rc) return rc;
@@ -441,7 +443,7 @@ static int32_t fit_blocks_impl(const float* x, const unsigned char* xq, const pt
     rc = plan_for(B, N, cfg->NP, cfg->D, &pl, true);
     if (rc) return rc;
     p.x = x; p.xq = xq; p.row_bytes = row_bytes;
-    p.lo = lo; p.hi = hi; p.block_index = block_index;
+    p.lo = lo; p.hi = hi; p.block_index = block_index; p.sel = sel;
     p.best = best; p.best_rss = best_rss; p.status = status; p.final_pop = final_pop; p.final_fit = final_fit;
     p.B = B; p.N = N; p.Npad = pl.Npad; p.NP = cfg->NP; p.NPpad = pl.NPpad; p.G = cfg->generations;
     p.fs = fs; p.t0 = cfg->t0; p.F = cfg->F;
@@ -514,6 +516,87 @@ int32_t pt_acquire(const float* x, int64_t B, int32_t N, double fs, int32_t D, c
     int dev_count = 0;
     if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0) { (void)cudaGetLastError(); set_error("no CUDA device"); return PT_ERR_CUDA; }
     if (acquire_launch(x, B, N, fs, D, acq, est, lo, hi, (cudaStream_t)stream)) return PT_ERR_CUDA;
+    return PT_OK;
+}
+
+static void refit_layout(int64_t B, size_t fit_ws, size_t* o_pb, size_t* o_tp, size_t* o_flags, size_t* o_list, size_t* o_fit,
+                         size_t* total) {
+    size_t off = 0;
+    auto take = [&off](size_t bytes) { size_t o = off; off += (bytes + 255) / 256 * 256; return o; };
+    *o_pb = take((size_t)B * 10 * 8); *o_tp = take((size_t)B * 8); *o_flags = take((size_t)B * 4); *o_list = take((size_t)B * 4);
+    *o_fit = take(fit_ws);
+    *total = off;
+}
+
+size_t pt_refit_doubtful_workspace_bytes(int64_t B, int32_t N, const pt_de_config* cfg) {
+    if (!cfg || B < 1) return 0;
+    size_t a, b, c, d, e, total;
+    refit_layout(B, pt_fit_blocks_workspace_bytes(B, N, cfg), &a, &b, &c, &d, &e, &total);
+    return total;
+}
+
+int32_t pt_refit_doubtful(const float* x, int64_t B, int32_t N, double fs, double* lo, double* hi, const uint32_t* block_index,
+                          const pt_de_config* cfg, const pt_retry_config* retry, double* best, float* best_rss,
+                          uint32_t* status, int32_t* attempts, void* workspace, size_t workspace_bytes, void* stream) {
+    if (!x || !lo || !hi || !best || !best_rss || !status || !attempts || !retry) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    int rc = check_cfg(cfg);
+    if (rc) return rc;
+    rc = check_common(B, N, fs, cfg->NP, cfg->D);
+    if (rc) return rc;
+    if (!(retry->phi_tol > 0.0) || !(retry->F_tol > 0.0) || retry->max_attempts < 0 || retry->max_attempts > 16 ||
+        !(retry->grow >= 1.0) || !(retry->f_floor >= 0.0) || !(retry->fdot_floor >= 0.0) || !(retry->a_rel >= 0.0) ||
+        !std::isfinite(retry->phi_tol + retry->F_tol + retry->grow + retry->f_floor + retry->fdot_floor + retry->a_rel)) {
+        set_error("invalid retry configuration");
+        return PT_ERR_INVALID_ARG;
+    }
+    const size_t fit_ws = pt_fit_blocks_workspace_bytes(B, N, cfg);
+    size_t o_pb, o_tp, o_flags, o_list, o_fit, total;
+    refit_layout(B, fit_ws, &o_pb, &o_tp, &o_flags, &o_list, &o_fit, &total);
+    if (!workspace || workspace_bytes < total) { set_error("pt_refit_doubtful needs %zu bytes of workspace, got %zu", total, workspace ? workspace_bytes : (size_t)0); return PT_ERR_UNSUPPORTED; }
+    if (reinterpret_cast<uintptr_t>(workspace) % 16) { set_error("workspace must be 16-byte aligned"); return PT_ERR_INVALID_ARG; }
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0) { (void)cudaGetLastError(); set_error("no CUDA device"); return PT_ERR_CUDA; }
+    unsigned char* ws = static_cast<unsigned char*>(workspace);
+    double* per_block = reinterpret_cast<double*>(ws + o_pb);
+    double* total_phase = reinterpret_cast<double*>(ws + o_tp);
+    uint32_t* flags = reinterpret_cast<uint32_t*>(ws + o_flags);
+    uint32_t* list = reinterpret_cast<uint32_t*>(ws + o_list);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int D = cfg->D;
+    const double T = (double)N / fs;
+    if (check_cuda(cudaMemsetAsync(attempts, 0, (size_t)B * sizeof(int32_t), st), "cudaMemsetAsync")) return PT_ERR_CUDA;
+    std::vector<uint32_t> h_flags((size_t)B), h_list;
+    auto flag_blocks = [&]() -> int {
+        if (doppler_launch(best, B, D, T, 0.0, nullptr, 0, per_block, total_phase, nullptr, st)) return PT_ERR_CUDA;
+        if (check_cuda(cudaGetLastError(), "doppler kernels launch")) return PT_ERR_CUDA;
+        if (retry_flag_launch(per_block, B, retry->phi_tol, retry->F_tol, flags, st)) return PT_ERR_CUDA;
+        if (check_cuda(cudaMemcpyAsync(h_flags.data(), flags, (size_t)B * 4, cudaMemcpyDeviceToHost, st), "D2H flags")) return PT_ERR_CUDA;
+        if (check_cuda(cudaStreamSynchronize(st), "pt_refit_doubtful")) return PT_ERR_CUDA;
+        h_list.clear();
+        for (int64_t b = 0; b < B; ++b)
+            if (h_flags[(size_t)b]) h_list.push_back((uint32_t)b);
+        return PT_OK;
+    };
+    double g = 1.0;
+    for (int a = 1; a <= retry->max_attempts; ++a, g *= retry->grow) {
+        rc = flag_blocks();
+        if (rc) return rc;
+        if (h_list.empty()) return PT_OK;
+        if (retry_box_launch(flags, best, lo, hi, B, D, T, g, retry, st)) return PT_ERR_CUDA;
+        if (check_cuda(cudaMemcpyAsync(list, h_list.data(), h_list.size() * 4, cudaMemcpyHostToDevice, st), "H2D list")) return PT_ERR_CUDA;
+        pt_de_config c = *cfg;
+        c.seed = cfg->seed + (uint64_t)a * 0x9E3779B97F4A7C15ull;
+        rc = fit_blocks_impl(x, nullptr, nullptr, 0, (int64_t)h_list.size(), N, fs, lo, hi, block_index, &c, best, best_rss, status,
+                             nullptr, nullptr, fit_ws ? ws + o_fit : nullptr, fit_ws, st, list);
+        if (rc) return rc;
+        if (retry_count_launch(list, (long long)h_list.size(), attempts, st)) return PT_ERR_CUDA;
+        // h_list is reused by the next attempt: the copy above must have been consumed
+        if (check_cuda(cudaStreamSynchronize(st), "pt_refit_doubtful")) return PT_ERR_CUDA;
+    }
+    rc = flag_blocks();
+    if (rc) return rc;
+    if (!h_list.empty() && retry->max_attempts > 0)
+        if (retry_abandon_launch(flags, B, status, st)) return PT_ERR_CUDA;
     return PT_OK;
 }
 

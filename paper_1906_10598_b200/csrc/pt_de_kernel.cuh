@@ -43,6 +43,7 @@ struct BlockParams {
     const double* lo;             // [B][D]  (fit)
     const double* hi;             // [B][D]  (fit)
     const uint32_t* block_index;  // [B] or null (fit)
+    const uint32_t* sel;          // [B] or null: when given, work item j of [blk0, B) is data block sel[j] (re-search of a subset)
     const float* pop_in;          // [B][NP][D] (fitness)
     float* fitness_out;           // [B][NP]    (fitness)
     double* best;                 // [B][D]
@@ -459,7 +460,8 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
         return (double)v;
     };
 
-    for (long long blk = p.blk0 + first_blk; blk < p.B; blk += blk_stride) {
+    for (long long item = p.blk0 + first_blk; item < p.B; item += blk_stride) {
+        const long long blk = p.sel ? (long long)p.sel[item] : item;
         const bool quantised = p.q.bits != 0;
         const float* xg = quantised ? nullptr : p.x + blk * (long long)p.N + n_lo;      // this CTA's slice of the block
         const unsigned char* xqrow = quantised ? p.xq + blk * p.row_bytes : nullptr;

@@ -16,6 +16,13 @@ int doppler_launch(const double* best, long long B, int D, double T, double los_
 int acquire_launch(const float* x, long long B, int N, double fs, int D, const pt_acq_config* a, double* est, double* lo,
                    double* hi, cudaStream_t st);
 
+// pt_retry.cu
+int retry_flag_launch(const double* per_block, long long B, double phi_tol, double F_tol_hz, uint32_t* flags, cudaStream_t st);
+int retry_box_launch(const uint32_t* flags, const double* best, double* lo, double* hi, long long B, int D, double T, double g,
+                     const pt_retry_config* rc, cudaStream_t st);
+int retry_count_launch(const uint32_t* sel, long long n, int32_t* attempts, cudaStream_t st);
+int retry_abandon_launch(const uint32_t* flags, long long B, uint32_t* status, cudaStream_t st);
+
 // pt_probe.cu
 int peak_probe(int kind, double* ops_per_s);
 

@@ -50,6 +50,13 @@ class AcqConfig(C.Structure):
                 ("fdot_bins", C.c_double), ("a_rel", C.c_double), ("a1_rel", C.c_double), ("fddot_hw", C.c_double)]
 
 
+class RetryConfig(C.Structure):
+    """Mirror of ``pt_retry_config`` (include/pt.h)."""
+
+    _fields_ = [("phi_tol", C.c_double), ("F_tol", C.c_double), ("max_attempts", C.c_int32), ("grow", C.c_double),
+                ("f_floor", C.c_double), ("fdot_floor", C.c_double), ("a_rel", C.c_double)]
+
+
 def lib():
     """Load (building first if needed) the CUDA library.  Raises if that is impossible."""
     global _lib
@@ -80,6 +87,10 @@ def lib():
     L.pt_track_host_q.restype = i32
     L.pt_acquire.argtypes = [p, i64, i32, f64, i32, C.POINTER(AcqConfig), p, p, p, p]
     L.pt_acquire.restype = i32
+    L.pt_refit_doubtful_workspace_bytes.argtypes = [i64, i32, C.POINTER(DEConfig)]
+    L.pt_refit_doubtful_workspace_bytes.restype = sz
+    L.pt_refit_doubtful.argtypes = [p, i64, i32, f64, p, p, p, C.POINTER(DEConfig), C.POINTER(RetryConfig), p, p, p, p, p, sz, p]
+    L.pt_refit_doubtful.restype = i32
     L.pt_fit_blocks_plan.argtypes = [i64, i32, C.POINTER(DEConfig), p]
     L.pt_fit_blocks_plan.restype = i32
     L.pt_doppler_products.argtypes = [p, i64, i32, f64, f64, p, i32, p, p, p, p]
@@ -229,6 +240,30 @@ def pt_acquire(x: torch.Tensor, fs: float, D: int, acq: AcqConfig) -> dict:
                           hi.data_ptr(), _stream())
     _check(rc, "pt_acquire")
     return {"est": est, "lo": lo, "hi": hi}
+
+
+def make_retry_config(*, phi_tol: float, F_tol: float, max_attempts: int = 3, grow: float = 2.0, f_floor: float = 1.0,
+                      fdot_floor: float = 1.0, a_rel: float = 0.1) -> RetryConfig:
+    return RetryConfig(float(phi_tol), float(F_tol), int(max_attempts), float(grow), float(f_floor), float(fdot_floor),
+                       float(a_rel))
+
+
+def pt_refit_doubtful(x: torch.Tensor, fs: float, lo: torch.Tensor, hi: torch.Tensor, cfg: DEConfig, retry: RetryConfig,
+                      fit: dict, *, block_index: torch.Tensor | None = None) -> torch.Tensor:
+    """Continuity check + re-search of doubtful blocks; updates lo, hi and fit["best"/"best_rss"/"status"] in place and
+    returns attempts[B] int32."""
+    B, N = x.shape
+    attempts = torch.empty(B, dtype=torch.int32, device=x.device)
+    ws_bytes = lib().pt_refit_doubtful_workspace_bytes(B, N, C.byref(cfg))
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=x.device)
+    bidx = None if block_index is None else _dev(block_index, torch.int32, "block_index")
+    rc = lib().pt_refit_doubtful(_dev(x, torch.float32, "x"), B, N, float(fs), _dev(lo, torch.float64, "lo"),
+                                 _dev(hi, torch.float64, "hi"), bidx, C.byref(cfg), C.byref(retry),
+                                 _dev(fit["best"], torch.float64, "best"), _dev(fit["best_rss"], torch.float32, "best_rss"),
+                                 _dev(fit["status"], torch.int32, "status"), attempts.data_ptr(), ws.data_ptr(), ws_bytes,
+                                 _stream())
+    _check(rc, "pt_refit_doubtful")
+    return attempts
 
 
 def pt_fit_blocks_plan(B: int, N: int, cfg: DEConfig) -> dict:
