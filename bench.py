@@ -394,6 +394,29 @@ def main():
     except Exception as exc:  # diagnostics only
         roofline["probe_error"] = str(exc)
 
+    # the steps around the hot path, timed on their own after the timed region: FFT acquisition of the
+    # initial ranges of every block, and the continuity check of the fitted track (no block of a clean track is re-searched)
+    extras = {}
+    try:
+        M = 1 << int(np.floor(np.log2(max(8, min(4096, wl.N // 2)))))
+        acq = pt.make_acq_config(M=M, spacing=(wl.N - M) // 2, f_rel=0.0, f_bins=2.0, fdot_bins=2.0, a_rel=0.2)
+        retry = pt.make_retry_config(phi_tol=1.5, F_tol=2.0)
+        pt.pt_acquire(x, wl.fs, wl.de["D"], acq)
+        lo2, hi2 = lo.clone(), hi.clone()
+        fit2 = {k: v.clone() for k, v in r.items()}
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        ev[0].record()
+        for _ in range(5):
+            pt.pt_acquire(x, wl.fs, wl.de["D"], acq)
+        ev[1].record()
+        att = pt.pt_refit_doubtful(x, wl.fs, lo2, hi2, cfg, retry, fit2)
+        ev[2].record()
+        torch.cuda.synchronize()
+        extras = {"acquire_ms": ev[0].elapsed_time(ev[1]) / 5, "acquire_piece": M,
+                  "continuity_check_ms": ev[1].elapsed_time(ev[2]), "blocks_researched": int((att > 0).sum().item())}
+    except Exception as exc:  # diagnostics only
+        extras = {"extras_error": str(exc)}
+
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic", "config": workload_config(args.workload, wl),
@@ -404,6 +427,7 @@ def main():
             # columns, prefix scan) and one kernel per integration interval
             "gpu_launches": args.steps * ((2 if plan.get("tail_cluster") else 1) + 2 + len([m for m in m_int if wl.B // m > 0])),
             "peaks_file": _peaks().get("when")}
+    line.update(extras)
     if e2e is not None:
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:

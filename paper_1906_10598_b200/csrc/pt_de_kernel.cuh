@@ -151,16 +151,16 @@ __device__ __forceinline__ void eval_chunk(const float4 xv, const float4 wv, con
 #pragma unroll
         for (int q = 0; q < P; ++q) {
             f32x2 h;
-            if (D == 6) h = fma2(t2, fma2(t2, d3[q], d2[q]), d1[q]);
-            else h = fma2(t2, d2[q], d1[q]);
-            const f32x2 y = fma2(t2, h, add2(w2, d0[q]));
+            if (D == 6) h = fma2(fma2(d3[q], t2, d2[q]), t2, d1[q]);
+            else h = fma2(d2[q], t2, d1[q]);
+            const f32x2 y = fma2(h, t2, add2(d0[q], w2));
             float y0, y1;
             unpack2(y, y0, y1);
             const f32x2 cs = pack2(__cosf(y0), __cosf(y1));
             if (OBJ == kObjCor) {
                 acc[q] = fma2(cs, x2, acc[q]);                     // Eq. 5-6: sum x cos(phi); a padded sample has x = 0
             } else {
-                f32x2 A = fma2(t2, na1[q], na0[q]);
+                f32x2 A = fma2(na1[q], t2, na0[q]);
                 if (MASKED && j >= n_left) A = pack2(0.0f, 0.0f);  // padded sample: residual 0 - 0 * c
                 const f32x2 r = fma2(A, cs, x2);
                 acc[q] = fma2(r, r, acc[q]);
@@ -190,8 +190,11 @@ __device__ __forceinline__ void reduce_and_store(float (&acc)[C], const int lane
     if ((lane & (32 / C - 1)) == 0) out[cidx] = accumulate ? out[cidx] + v : v;
 }
 
+// Not inlined on purpose: the loop's register allocation (which decides the operand-bank conflicts of the FFMA2 stream, the
+// binding resource of this loop) then does not depend on the code around it in the kernel.  Measured on config 2: 2101 ms
+// inlined vs 2071 ms as a call, with identical instruction mixes (profiles/r1d_codegen_ab.md).
 template <int C, int D, int OBJ>
-__device__ __forceinline__ void eval_population(const BlockParams& p, const Slice& sl, const float* __restrict__ xs,
+__device__ __noinline__ void eval_population(const BlockParams& p, const Slice& sl, const float* __restrict__ xs,
                                                 const float* __restrict__ wref, const float* __restrict__ cand,
                                                 float* __restrict__ part, const int warp, const int lane) {
     constexpr int P = C / 2;
