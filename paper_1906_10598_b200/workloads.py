@@ -350,3 +350,38 @@ def quantise(x: np.ndarray, bits: int):
     shifts = (np.arange(per) * bits).astype(np.uint16)
     xq = np.bitwise_or.reduce(fields << shifts, axis=-1).astype(np.uint8)
     return np.ascontiguousarray(xq), dict(bits=bits, is_signed=False, scale=step, offset=offset)
+
+
+# ------------------------------------------------------------------------------------------
+# Paper-shaped blocks (PAPER.md:51 footnote 2 "the data block is usually 2 seconds and sampling is 200KHz"; :94 "the
+# data block size is about 400K ... evaluated by the DE solver ~80,000 times"; Table 4: Dim_XC 6, itermax 200, F_XC 0.5,
+# CR_XC 0.85, strategy 3).  NP = 400 = 80,000 / 200.  Stand-in for the Mars Express recording the paper times.
+# ------------------------------------------------------------------------------------------
+def paper_blocks(B: int = 148, case: int = 0, N: int = 400000, fs: float = 200000.0, snr_db: float = -13.0) -> Workload:
+    """B independent 2 s blocks of 400 000 samples at 200 kHz: a0~U(0.8,1.2), a1~U(-0.02,0.02), phi0~U(-pi,pi),
+    f~U(20,80) kHz, fdot~U(-30,30) Hz/s, fddot~U(-0.5,0.5) Hz/s^2; -13 dB per sample = 40 dB-Hz.  Boxes are of the
+    run-time (tracking) kind: phi0 a full turn, f +-2/T, fdot +-4/T^2, fddot +-16/T^3 about the
+    truth, a0 +-10 %, a1 +-0.2 a0/T."""
+    T = N / fs
+    t = -T / 2.0 + np.arange(N, dtype=np.float64) / fs
+    x = np.empty((B, N), dtype=np.float32)
+    truth = np.empty((B, 6), dtype=np.float64)
+    sig = np.empty(B)
+    for k in range(B):
+        rng = np.random.default_rng([BASE_SEED + 5000 + int(case), k])
+        a0, a1 = rng.uniform(0.8, 1.2), rng.uniform(-0.02, 0.02)
+        phi0, f = rng.uniform(-np.pi, np.pi), rng.uniform(20e3, 80e3)
+        fdot, fddot = rng.uniform(-30.0, 30.0), rng.uniform(-0.5, 0.5)
+        truth[k] = (a0, a1, phi0, f, fdot, fddot)
+        sig[k] = _noise_sigma(a0, snr_db)
+        ph = phi0 + 2.0 * np.pi * (f * t + fdot * t * t / 2.0 + fddot * t**3 / 6.0)
+        x[k] = ((a0 + a1 * t) * np.cos(ph) + sig[k] * rng.standard_normal(N)).astype(np.float32)
+    lo, hi = truth.copy(), truth.copy()
+    hw = np.array([0.0, 0.0, 0.0, 2.0 / T, 4.0 / T**2, 16.0 / T**3])
+    lo -= hw; hi += hw
+    lo[:, 0], hi[:, 0] = 0.9 * truth[:, 0], 1.1 * truth[:, 0]
+    lo[:, 1], hi[:, 1] = -0.2 * truth[:, 0] / T, 0.2 * truth[:, 0] / T
+    lo[:, 2], hi[:, 2] = -np.pi, np.pi
+    de = dict(NP=400, D=6, generations=200, F=0.5, CR=0.85, strategy=3)
+    return Workload(name="paper_blocks", config=5, x=x, fs=float(fs), truth=truth, lo=lo, hi=hi, sigma=float(np.mean(sig)),
+                    de=de, block_index=np.arange(B, dtype=np.uint32), meta={"sigma_per_block": sig, "box": "tracking"})

@@ -143,3 +143,34 @@ def test_invalid_quant_is_rejected(pt):
         pt.pt_fit_blocks(_cuda(xq[:, :500]), wl.fs, _cuda(wl.lo), _cuda(wl.hi), cfg, quant=pt.make_quant(8, True, 1.0), N=wl.N)
     with pytest.raises(pt.PtError):
         pt.pt_unpack_samples(_cuda(xq), wl.N, pt.make_quant(8, True, float("nan")))
+
+
+def test_paper_shaped_blocks(pt):
+    """PAPER.md:51, :94, Table 4: 400 000 samples (2 s at 200 kHz), D = 6, strategy 3, F 0.5, CR 0.85, 200 iterations,
+    NP = 400 (80 000 evaluations), 16-bit samples (Table 3), streamed through shared memory.  In bench.py's launch
+    configuration on 4 blocks: every result is valid (its RSS is the oracle's objective at its own parameters), the
+    chi^2 sits at the noise floor, phi0 and f land within 4 Cramer-Rao sigma of the truth."""
+    wl = W.paper_blocks(B=4)
+    xq, qd = W.quantise(wl.x, 16)
+    q = pt.make_quant(qd["bits"], qd["is_signed"], qd["scale"], qd["offset"])
+    de = wl.de
+    cfg = pt.make_config(D=6, NP=de["NP"], generations=de["generations"], F=de["F"], CR=de["CR"], seed=1, t0=wl.t0,
+                         strategy=de["strategy"])
+    with _forced_cluster(1):
+        assert pt.pt_fit_blocks_plan(148, wl.N, cfg)["resident"] == 0
+        g = pt.pt_fit_blocks(_cuda(xq), wl.fs, _cuda(wl.lo), _cuda(wl.hi), cfg, quant=q, N=wl.N)
+    g = {k: v.cpu().numpy() for k, v in g.items()}
+    x = oracle.unpack_samples(xq, wl.N, 16, True, qd["scale"], qd["offset"])
+    for k in range(wl.B):
+        assert abs(g["best_rss"][k] - oracle.rss(x[k], wl.fs, g["best"][k])) < 1e-4 * g["best_rss"][k]
+        s2 = wl.meta["sigma_per_block"][k] ** 2
+        assert abs(g["best_rss"][k] - (wl.N - 6) * s2) < 5 * s2 * np.sqrt(2.0 * wl.N)
+        # Cramer-Rao bounds from the Fisher matrix of Eq. 2 in white noise
+        t = wl.t0 + np.arange(wl.N) / wl.fs
+        th = wl.truth[k]
+        ph = th[2] + 2 * np.pi * (th[3] * t + th[4] * t * t / 2 + th[5] * t**3 / 6)
+        A, c, sn = th[0] + th[1] * t, np.cos(ph), np.sin(ph)
+        J = np.array([c, t * c, -A * sn, -A * sn * 2 * np.pi * t, -A * sn * np.pi * t * t, -A * sn * np.pi * t**3 / 3])
+        sd = np.sqrt(np.diag(np.linalg.inv(J @ J.T / s2)))
+        assert abs(_wrap(g["best"][k, 2] - wl.truth[k, 2])) < 4 * sd[2] + 1e-3
+        assert abs(g["best"][k, 3] - wl.truth[k, 3]) < 4 * sd[3]
