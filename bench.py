@@ -36,7 +36,7 @@ XU_LANES_PER_SM = 16            # MUFU lanes per SM (4 per sub-partition): one c
 SM_MAX_MHZ = 1965.0
 XU_PEAK = SM_COUNT * XU_LANES_PER_SM * SM_MAX_MHZ * 1e6     # 4.65e12 sample-evaluations/s, DESIGN.md "Roofline"
 # dram__bytes_read.sum + dram__bytes_write.sum of one pt_block_kernel launch, from the ncu capture in profiles/
-TRAFFIC_BYTES_PER_LAUNCH = {"config2": 2.50e8}     # profiles/r1b_bench_launches.md (main + tail launch of one step)
+TRAFFIC_BYTES_PER_LAUNCH = {"config2": 2.44e8}     # profiles/r1e_bench_launches.md (main + tail launch of one step, reads)
 
 
 def _peaks():
