@@ -278,6 +278,19 @@ PT_API int32_t pt_track_host_q(const void* xq, const pt_quant* quant, int64_t ro
                         uint32_t* status, double* per_block, double* total_phase, double* const* interval_out);
 
 /*
+ * pt_track_auto_host -- the paper's whole process flow (section 3.1.4) on HOST buffers, with no
+ * caller-supplied ranges: copy x to the device, pt_acquire (initial ranges), pt_fit_blocks, pt_refit_doubtful when
+ * `retry` is not NULL (continuity check and re-search), pt_doppler_products, copy the results back; synchronous.
+ * Every pointer is a [host] pointer; outputs that are NULL are skipped.  lo, hi [B][D] out: the ranges finally used;
+ * attempts [B] int32 out (only with retry).  Results are identical to calling the four device entry points in turn.
+ */
+PT_API int32_t pt_track_auto_host(const float* x, int64_t B, int32_t N, double fs, const pt_de_config* cfg,
+                           const pt_acq_config* acq, const pt_retry_config* retry, double los_scale,
+                           const int32_t* blocks_per_interval, int32_t n_intervals, double* lo, double* hi, double* best,
+                           float* best_rss, uint32_t* status, int32_t* attempts, double* per_block, double* total_phase,
+                           double* const* interval_out);
+
+/*
  * pt_de_draws -- debug/parity entry: the integer random draws the DE kernel uses, for Q queries.
  * query  [Q][3]  u32 device: (block_index, generation >= 1, candidate)
  * out    [Q][5]  i32 device: r1, r2, r3, jrand, crossover mask (bit j set = coordinate j takes the mutant)

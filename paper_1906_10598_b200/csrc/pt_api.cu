@@ -650,8 +650,12 @@ int32_t pt_peak_probe(int32_t kind, double* ops_per_s) {
 static int32_t track_host_impl(const float* x, const void* xq, const pt_quant* quant, int64_t row_bytes, int64_t B, int32_t N,
                                double fs, const double* lo, const double* hi, const pt_de_config* cfg, double los_scale,
                                const int32_t* blocks_per_interval, int32_t n_intervals, double* best, float* best_rss,
-                               uint32_t* status, double* per_block, double* total_phase, double* const* interval_out) {
-    if ((!x && !xq) || !lo || !hi) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+                               uint32_t* status, double* per_block, double* total_phase, double* const* interval_out,
+                               const pt_acq_config* acq = nullptr, const pt_retry_config* retry = nullptr,
+                               double* lo_out = nullptr, double* hi_out = nullptr, int32_t* attempts = nullptr) {
+    // acq != null: the ranges come from pt_acquire (lo, hi are not read); retry != null: pt_refit_doubtful after the fit
+    if ((!x && !xq) || (!acq && (!lo || !hi))) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    if ((acq || retry) && xq) { set_error("acquisition and re-search take fp32 samples"); return PT_ERR_UNSUPPORTED; }
     if (xq) {
         Quant qq;
         const int rq = check_quant(quant, row_bytes, N, &qq);
@@ -662,7 +666,7 @@ static int32_t track_host_impl(const float* x, const void* xq, const pt_quant* q
     rc = check_common(B, N, fs, cfg->NP, cfg->D);
     if (rc) return rc;
     if (n_intervals < 0 || (n_intervals > 0 && (!blocks_per_interval || !interval_out))) { set_error("invalid interval arguments"); return PT_ERR_INVALID_ARG; }
-    for (long long k = 0; k < B * cfg->D; ++k)
+    for (long long k = 0; !acq && k < B * cfg->D; ++k)
         if (!(lo[k] <= hi[k])) { set_error("lo > hi at element %lld", k); return PT_ERR_INVALID_ARG; }
     const int D = cfg->D;
     const size_t nx = xq ? (size_t)B * (size_t)row_bytes : (size_t)B * N * sizeof(float), nbox = (size_t)B * D * sizeof(double);
@@ -673,6 +677,9 @@ static int32_t track_host_impl(const float* x, const void* xq, const pt_quant* q
     const size_t o_rss = take((size_t)B * 4), o_st = take((size_t)B * 4), o_pb = take((size_t)B * 10 * 8), o_tp = take((size_t)B * 8);
     const size_t ws_bytes = pt_fit_blocks_workspace_bytes(B, N, cfg);
     const size_t o_ws = take(ws_bytes);
+    const size_t o_est = take(acq ? (size_t)B * 8 * 8 : 0), o_att = take(retry ? (size_t)B * 4 : 0);
+    const size_t rws_bytes = retry ? pt_refit_doubtful_workspace_bytes(B, N, cfg) : 0;
+    const size_t o_rws = take(rws_bytes);
     std::vector<size_t> o_iv(n_intervals);
     std::vector<long long> cnt(n_intervals);
     for (int k = 0; k < n_intervals; ++k) {
@@ -689,14 +696,28 @@ static int32_t track_host_impl(const float* x, const void* xq, const pt_quant* q
     for (int k = 0; k < n_intervals; ++k) d_iv[k] = reinterpret_cast<double*>(arena + o_iv[k]);
     do {
         if (check_cuda(cudaMemcpyAsync(arena + o_x, xq ? xq : static_cast<const void*>(x), nx, cudaMemcpyHostToDevice, st), "H2D x")) { ret = PT_ERR_CUDA; break; }
-        if (check_cuda(cudaMemcpyAsync(arena + o_lo, lo, nbox, cudaMemcpyHostToDevice, st), "H2D lo")) { ret = PT_ERR_CUDA; break; }
-        if (check_cuda(cudaMemcpyAsync(arena + o_hi, hi, nbox, cudaMemcpyHostToDevice, st), "H2D hi")) { ret = PT_ERR_CUDA; break; }
+        if (acq) {
+            ret = pt_acquire(reinterpret_cast<float*>(arena + o_x), B, N, fs, D, acq, reinterpret_cast<double*>(arena + o_est),
+                             reinterpret_cast<double*>(arena + o_lo), reinterpret_cast<double*>(arena + o_hi), st);
+            if (ret) break;
+        } else {
+            if (check_cuda(cudaMemcpyAsync(arena + o_lo, lo, nbox, cudaMemcpyHostToDevice, st), "H2D lo")) { ret = PT_ERR_CUDA; break; }
+            if (check_cuda(cudaMemcpyAsync(arena + o_hi, hi, nbox, cudaMemcpyHostToDevice, st), "H2D hi")) { ret = PT_ERR_CUDA; break; }
+        }
         ret = fit_blocks_impl(xq ? nullptr : reinterpret_cast<float*>(arena + o_x), xq ? arena + o_x : nullptr, quant, row_bytes, B,
                               N, fs, reinterpret_cast<double*>(arena + o_lo), reinterpret_cast<double*>(arena + o_hi), nullptr,
                               cfg, reinterpret_cast<double*>(arena + o_best), reinterpret_cast<float*>(arena + o_rss),
                               reinterpret_cast<uint32_t*>(arena + o_st), nullptr, nullptr, ws_bytes ? arena + o_ws : nullptr,
                               ws_bytes, st);
         if (ret) break;
+        if (retry) {
+            ret = pt_refit_doubtful(reinterpret_cast<float*>(arena + o_x), B, N, fs, reinterpret_cast<double*>(arena + o_lo),
+                                    reinterpret_cast<double*>(arena + o_hi), nullptr, cfg, retry,
+                                    reinterpret_cast<double*>(arena + o_best), reinterpret_cast<float*>(arena + o_rss),
+                                    reinterpret_cast<uint32_t*>(arena + o_st), reinterpret_cast<int32_t*>(arena + o_att),
+                                    arena + o_rws, rws_bytes, st);
+            if (ret) break;
+        }
         ret = pt_doppler_products(reinterpret_cast<double*>(arena + o_best), B, D, (double)N / fs, los_scale,
                                   blocks_per_interval, n_intervals, reinterpret_cast<double*>(arena + o_pb),
                                   reinterpret_cast<double*>(arena + o_tp), d_iv.data(), st);
@@ -707,6 +728,9 @@ static int32_t track_host_impl(const float* x, const void* xq, const pt_quant* q
         if (e == cudaSuccess && status) e = cudaMemcpyAsync(status, arena + o_st, (size_t)B * 4, cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess && per_block) e = cudaMemcpyAsync(per_block, arena + o_pb, (size_t)B * 80, cudaMemcpyDeviceToHost, st);
         if (e == cudaSuccess && total_phase) e = cudaMemcpyAsync(total_phase, arena + o_tp, (size_t)B * 8, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && lo_out) e = cudaMemcpyAsync(lo_out, arena + o_lo, nbox, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && hi_out) e = cudaMemcpyAsync(hi_out, arena + o_hi, nbox, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && attempts && retry) e = cudaMemcpyAsync(attempts, arena + o_att, (size_t)B * 4, cudaMemcpyDeviceToHost, st);
         for (int k = 0; k < n_intervals && e == cudaSuccess; ++k)
             if (cnt[k] > 0 && interval_out[k])
                 e = cudaMemcpyAsync(interval_out[k], arena + o_iv[k], (size_t)cnt[k] * 16, cudaMemcpyDeviceToHost, st);
@@ -726,6 +750,15 @@ int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, const dou
     if (!x) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
     return track_host_impl(x, nullptr, nullptr, 0, B, N, fs, lo, hi, cfg, los_scale, blocks_per_interval, n_intervals, best,
                            best_rss, status, per_block, total_phase, interval_out);
+}
+
+int32_t pt_track_auto_host(const float* x, int64_t B, int32_t N, double fs, const pt_de_config* cfg, const pt_acq_config* acq,
+                           const pt_retry_config* retry, double los_scale, const int32_t* blocks_per_interval,
+                           int32_t n_intervals, double* lo, double* hi, double* best, float* best_rss, uint32_t* status,
+                           int32_t* attempts, double* per_block, double* total_phase, double* const* interval_out) {
+    if (!x || !acq) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    return track_host_impl(x, nullptr, nullptr, 0, B, N, fs, nullptr, nullptr, cfg, los_scale, blocks_per_interval, n_intervals,
+                           best, best_rss, status, per_block, total_phase, interval_out, acq, retry, lo, hi, attempts);
 }
 
 int32_t pt_track_host_q(const void* xq, const pt_quant* quant, int64_t row_bytes, int64_t B, int32_t N, double fs,

@@ -91,6 +91,9 @@ def lib():
     L.pt_refit_doubtful_workspace_bytes.restype = sz
     L.pt_refit_doubtful.argtypes = [p, i64, i32, f64, p, p, p, C.POINTER(DEConfig), C.POINTER(RetryConfig), p, p, p, p, p, sz, p]
     L.pt_refit_doubtful.restype = i32
+    L.pt_track_auto_host.argtypes = [p, i64, i32, f64, C.POINTER(DEConfig), C.POINTER(AcqConfig), C.POINTER(RetryConfig), f64, p,
+                                     i32, p, p, p, p, p, p, p, p, p]
+    L.pt_track_auto_host.restype = i32
     L.pt_fit_blocks_plan.argtypes = [i64, i32, C.POINTER(DEConfig), p]
     L.pt_fit_blocks_plan.restype = i32
     L.pt_doppler_products.argtypes = [p, i64, i32, f64, f64, p, i32, p, p, p, p]
@@ -320,6 +323,35 @@ def pt_track_host(x, fs: float, lo, hi, cfg: DEConfig, los_scale: float = 0.0, b
     _check(rc, "pt_track_host")
     return {"best": best, "best_rss": best_rss, "status": status, "per_block": per_block, "total_phase": total,
             "intervals": outs}
+
+
+def pt_track_auto_host(x, fs: float, cfg: DEConfig, acq: AcqConfig, retry: RetryConfig | None = None,
+                       los_scale: float = 0.0, blocks_per_interval=()):
+    """The whole process flow on HOST tensors with no caller ranges: H2D, acquisition, fit, re-search (if ``retry``),
+    products, D2H."""
+    B, N = x.shape
+    D = cfg.D
+    if x.is_cuda or x.dtype != torch.float32 or not x.is_contiguous():
+        raise PtError("x must be a contiguous host tensor of dtype float32")
+    m = [int(v) for v in blocks_per_interval]
+    lo = torch.empty((B, D), dtype=torch.float64)
+    hi = torch.empty((B, D), dtype=torch.float64)
+    best = torch.empty((B, D), dtype=torch.float64)
+    best_rss = torch.empty(B, dtype=torch.float32)
+    status = torch.empty(B, dtype=torch.int32)
+    attempts = torch.zeros(B, dtype=torch.int32)
+    per_block = torch.empty((B, 10), dtype=torch.float64)
+    total = torch.empty(B, dtype=torch.float64)
+    outs = [torch.empty((B // v, 2), dtype=torch.float64) for v in m]
+    m_arr = (C.c_int32 * max(len(m), 1))(*m)
+    ptrs = (C.c_void_p * max(len(m), 1))(*[o.data_ptr() if o.numel() else None for o in outs])
+    rc = lib().pt_track_auto_host(x.data_ptr(), B, N, float(fs), C.byref(cfg), C.byref(acq),
+                                  C.byref(retry) if retry is not None else None, float(los_scale), m_arr, len(m),
+                                  lo.data_ptr(), hi.data_ptr(), best.data_ptr(), best_rss.data_ptr(), status.data_ptr(),
+                                  attempts.data_ptr(), per_block.data_ptr(), total.data_ptr(), ptrs)
+    _check(rc, "pt_track_auto_host")
+    return {"lo": lo, "hi": hi, "best": best, "best_rss": best_rss, "status": status, "attempts": attempts,
+            "per_block": per_block, "total_phase": total, "intervals": outs}
 
 
 def pt_de_draws(query: torch.Tensor, NP: int, D: int, CR: float, seed: int) -> torch.Tensor:

@@ -107,3 +107,37 @@ def test_invalid_acquisition_arguments(pt):
                dict(M=256, spacing=100, f_rel=-1.0)):
         with pytest.raises(pt.PtError):
             pt.pt_acquire(_cuda(wl.x), wl.fs, 5, pt.make_acq_config(**kw))
+
+
+def test_track_auto_host_is_the_composition_of_the_device_calls(pt):
+    """pt_track_auto_host (PAPER.md:250-252 process flow on host buffers: acquisition -> fit -> continuity check and
+    re-search -> products) gives bit-identical results to the four device entry points called in turn."""
+    wl = W.config1(blocks=range(10), generations=150, NP=40)
+    x = wl.x.copy()
+    x[6] = (wl.sigma * np.random.default_rng(3).standard_normal(wl.N)).astype(np.float32)     # the carrier drops out
+    M = 2048
+    acq = pt.make_acq_config(M=M, spacing=(wl.N - M) // 2, f_rel=0.0, f_bins=2.0, fdot_bins=2.0, a_rel=0.2)
+    retry = pt.make_retry_config(phi_tol=0.5, F_tol=0.5, f_floor=2.0, fdot_floor=2.0)
+    cfg = pt.make_config(D=5, NP=40, generations=150, seed=8, t0=wl.t0)
+    h = pt.pt_track_auto_host(torch.from_numpy(x), wl.fs, cfg, acq, retry, 0.0, [2, 5])
+    xd = _cuda(x)
+    r = pt.pt_acquire(xd, wl.fs, 5, acq)
+    fit = pt.pt_fit_blocks(xd, wl.fs, r["lo"], r["hi"], cfg)
+    att = pt.pt_refit_doubtful(xd, wl.fs, r["lo"], r["hi"], cfg, retry, fit)
+    per_block, total, ivs = pt.pt_doppler_products(fit["best"], wl.T, 0.0, [2, 5])
+    assert np.array_equal(h["best"].numpy(), fit["best"].cpu().numpy())
+    assert np.array_equal(h["status"].numpy(), fit["status"].cpu().numpy())
+    assert np.array_equal(h["attempts"].numpy(), att.cpu().numpy())
+    assert np.array_equal(h["lo"].numpy(), r["lo"].cpu().numpy()) and np.array_equal(h["hi"].numpy(), r["hi"].cpu().numpy())
+    assert np.array_equal(h["total_phase"].numpy(), total.cpu().numpy())
+    assert np.array_equal(h["intervals"][1].numpy(), ivs[1].cpu().numpy())
+    # the dropped block is searched again (abandonment itself is covered by test_gpu_retry: here one of its borders may
+    # pass the check by chance); the rest of the track is solved without caller ranges
+    a = h["attempts"].numpy()
+    assert a[6] >= 1
+    ok = [b for b in range(10) if b != 6]
+    assert np.all((h["status"].numpy()[ok] & 4) == 0)
+    assert np.max(np.abs(h["best"].numpy()[ok, 3] - wl.truth[ok, 3])) < 0.02
+    # without retry the same call stops after the fit
+    h2 = pt.pt_track_auto_host(torch.from_numpy(x), wl.fs, cfg, acq, None, 0.0, [])
+    assert int(h2["attempts"].sum()) == 0
