@@ -174,7 +174,8 @@ def run_reference(args, rank: int, world: int):
     else:
         wl = W.config2(blocks=range(nb))
     wl = apply_variant(wl, args.strategy, args.objective)
-    G = min(wl.de["generations"], args.ref_generations)
+    # bounded sample per step: about 2e10 sample-evaluations at most (10-30 s on 16 cores)
+    G = int(max(2, min(wl.de["generations"], args.ref_generations, 2e10 * cores / 16 / (float(wl.B) * wl.de["NP"] * wl.N) - 1)))
     units = float(wl.B) * wl.de["NP"] * (G + 1) * wl.N
     times = []
     for it in range(args.warmup + args.steps):
