@@ -45,6 +45,7 @@ typedef enum {
 } pt_status;
 
 #define PT_MAX_NP 1024      /* population limit of the DE kernel                                  */
+#define PT_MAX_N 16777216   /* samples per block: the evaluation loop carries the sample index exactly in fp32 (2^24) */
 #define PT_PER_BLOCK_COLS 10 /* columns of pt_doppler_products' per_block output                  */
 
 /*

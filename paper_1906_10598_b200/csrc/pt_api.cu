@@ -282,6 +282,7 @@ static uint32_t cr32_of(double CR) {
 static int check_common(long long B, int N, double fs, int NP, int D) {
     if (B < 1) { set_error("B must be >= 1"); return PT_ERR_INVALID_ARG; }
     if (N < 8 || (N & 1)) { set_error("N must be even and >= 8 (got %d)", N); return PT_ERR_INVALID_ARG; }
+    if (N > PT_MAX_N) { set_error("N = %d exceeds PT_MAX_N = %d (sample indices are carried exactly in fp32)", N, PT_MAX_N); return PT_ERR_UNSUPPORTED; }
     if (!(fs > 0.0)) { set_error("fs must be > 0"); return PT_ERR_INVALID_ARG; }
     if (D != 5 && D != 6) { set_error("D must be 5 or 6 (got %d)", D); return PT_ERR_INVALID_ARG; }
     if (NP < 4) { set_error("NP must be >= 4 (got %d)", NP); return PT_ERR_INVALID_ARG; }

@@ -47,8 +47,10 @@ def test_header_compiles_as_plain_c(tmp_path):
 def test_struct_layouts_match_the_binding(tmp_path):
     """sizeof / offsetof of pt_de_config and pt_quant as gcc lays them out from include/pt.h = the ctypes mirrors."""
     import subprocess
-    from paper_1906_10598_b200.pt import DEConfig, Quant
-    fields = {"pt_de_config": [f for f, _ in DEConfig._fields_], "pt_quant": [f for f, _ in Quant._fields_]}
+    from paper_1906_10598_b200.pt import AcqConfig, DEConfig, Quant, RetryConfig
+    classes = (DEConfig, Quant, AcqConfig, RetryConfig)
+    fields = {"pt_de_config": [f for f, _ in DEConfig._fields_], "pt_quant": [f for f, _ in Quant._fields_],
+              "pt_acq_config": [f for f, _ in AcqConfig._fields_], "pt_retry_config": [f for f, _ in RetryConfig._fields_]}
     body = ['#include <stdio.h>', '#include <stddef.h>', '#include "pt.h"', 'int main(void){']
     for st, names in fields.items():
         body.append('printf("%%zu", sizeof(%s));' % st)
@@ -61,7 +63,7 @@ def test_struct_layouts_match_the_binding(tmp_path):
     exe = tmp_path / "layout"
     subprocess.run(["gcc", "-std=c99", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
     lines = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.strip().splitlines()
-    for line, (st, names), cls in zip(lines, fields.items(), (DEConfig, Quant)):
+    for line, (st, names), cls in zip(lines, fields.items(), classes):
         nums = [int(v) for v in line.split()]
         assert nums[0] == C.sizeof(cls), st
         assert nums[1:] == [getattr(cls, f).offset for f in names], st
@@ -90,6 +92,7 @@ def test_argument_validation_needs_no_gpu(lib_path):
     assert call(cfg=pt.make_config(D=5, NP=60, generations=1, F=2.5, t0=0.0)) == -1
     assert call(cfg=pt.make_config(D=5, NP=60, generations=1, CR=1.5, t0=0.0)) == -1
     assert call(cfg=pt.make_config(D=5, NP=4096, generations=1, t0=0.0)) == -2       # beyond PT_MAX_NP
+    assert call(N=(1 << 24) + 2) == -2                                                # beyond PT_MAX_N
     assert L.pt_fitness(dummy, 1, 1000, 1000.0, -0.5, dummy, 60, 7, dummy, None, 0, None) == -1
     assert L.pt_doppler_products(dummy, 0, 5, 1.0, 0.0, None, 0, dummy, dummy, None, None) == -1
     assert L.pt_doppler_products(dummy, 4, 5, -1.0, 0.0, None, 0, dummy, dummy, None, None) == -1
