@@ -64,11 +64,15 @@ def make_workload(name: str, case: int):
     raise SystemExit("unknown workload %s" % name)
 
 
-def apply_variant(wl, strategy: int, objective: str):
+def apply_variant(wl, strategy: int, objective: str, fix_a1: bool = False):
     """--strategy / --objective: the widened rows.  For the correlation objective the amplitude
     is fixed (Eq. 6): a0 = the profile's amplitude at the block centre, a1 = 0, zero-width boxes."""
     wl.de["strategy"] = int(strategy) if strategy else int(wl.de.get("strategy", 1))
     wl.de["objective"] = 1 if objective == "cor" else 0
+    if fix_a1:          # amplitude slope fixed at zero (PAPER.md:139): the kernel takes its constant-amplitude loop
+        wl.lo = wl.lo.copy(); wl.hi = wl.hi.copy()
+        wl.lo[:, 1] = wl.hi[:, 1] = 0.0
+        wl.meta["fix_a1"] = True
     if objective == "cor":
         wl.lo = wl.lo.copy(); wl.hi = wl.hi.copy()
         wl.lo[:, 0] = wl.hi[:, 0] = wl.truth[:, 0]
@@ -173,7 +177,7 @@ def run_reference(args, rank: int, world: int):
         wl = W.config2(blocks=range(2), generations=3)
     else:
         wl = W.config2(blocks=range(nb))
-    wl = apply_variant(wl, args.strategy, args.objective)
+    wl = apply_variant(wl, args.strategy, args.objective, args.fix_a1)
     # bounded sample per step: about 2e10 sample-evaluations at most (10-30 s on 16 cores)
     G = int(max(2, min(wl.de["generations"], args.ref_generations, 2e10 * cores / 16 / (float(wl.B) * wl.de["NP"] * wl.N) - 1)))
     units = float(wl.B) * wl.de["NP"] * (G + 1) * wl.N
@@ -251,7 +255,7 @@ def run_sweep(args, dev):
 
 def workload_config(name: str, wl, full=True) -> dict:
     return {"workload": "BASELINE.json config 2 (one-hour track)" if name == "config2" else name,
-            "strategy": wl.de.get("strategy", 1), "objective": "cor (Eq. 5-6)" if wl.de.get("objective", 0) else "chi2 (Eq. 4)",
+            "strategy": wl.de.get("strategy", 1), "a1": "fixed at 0" if wl.meta.get("fix_a1") else "free", "objective": "cor (Eq. 5-6)" if wl.de.get("objective", 0) else "chi2 (Eq. 4)",
             "blocks": wl.B if full else "%d (sample)" % wl.B, "samples_per_block": wl.N, "fs_hz": wl.fs,
             "NP": wl.de["NP"], "D": wl.de["D"], "generations": wl.de["generations"], "F": wl.de["F"], "CR": wl.de["CR"],
             "box": "tracking ranges (PAPER.md:191-197) about the truth" if wl.meta.get("box") == "tracking" else
@@ -269,6 +273,7 @@ def main():
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--ref-generations", type=int, default=100)
     ap.add_argument("--strategy", type=int, default=0, help="mutation strategy 1..6 (Table 4); 0 = the workload's own (DE/rand/1)")
+    ap.add_argument("--fix-a1", action="store_true", help="fix the amplitude slope at zero (a1 box [0, 0], PAPER.md:139)")
     ap.add_argument("--objective", default="chi2", choices=["chi2", "cor"], help="Eq. 4 (default) or Eq. 5-6")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -304,7 +309,7 @@ def main():
             raise SystemExit("--workload sweep is a 1-GPU report")
         run_sweep(args, dev)
         return
-    wl = apply_variant(make_workload(args.workload, case=rank), args.strategy, args.objective)   # every rank fits its own track
+    wl = apply_variant(make_workload(args.workload, case=rank), args.strategy, args.objective, args.fix_a1)   # every rank fits its own track
     cfg = pt.make_config(D=wl.de["D"], NP=wl.de["NP"], generations=wl.de["generations"], F=wl.de["F"], CR=wl.de["CR"],
                          seed=1 + rank, t0=wl.t0, strategy=wl.de["strategy"], objective=wl.de["objective"])
     plan = pt.pt_fit_blocks_plan(wl.B, wl.N, cfg)
@@ -394,7 +399,8 @@ def main():
                 "MEASURED_PEAKS.json holds no ALU peak",
                 "frac_at_sampled_clock": achieved / (SM_COUNT * XU_LANES_PER_SM * sm_mhz * 1e6),
                 # algorithmic flops per sample-evaluation: chi^2 5 (D=5) / 6 FMA; correlation 3 / 4 FMA
-                "fp32_flops_achieved_tflops": achieved * ((10 if wl.de["D"] == 5 else 12) - (4 if wl.de["objective"] else 0)) / 1e12}
+                "fp32_flops_achieved_tflops": achieved * ((10 if wl.de["D"] == 5 else 12) - (4 if wl.de["objective"] else
+                                                            (2 if wl.meta.get("fix_a1") else 0))) / 1e12}
     try:
         roofline["measured_mufu_peak"] = pt.pt_peak_probe(1) / 1e12
         roofline["measured_ffma_peak_tflops"] = 2 * pt.pt_peak_probe(0) / 1e12

@@ -34,6 +34,10 @@ enum Mode { kModeFit = 0, kModeFitness = 1 };
 //     F_cor = 1 / (arctan(cor) + pi/2),  cor = sum_n x_n a0 cos(phi(t_n))       (constant amplitude a0, a1 unused).
 // F_cor is strictly decreasing in cor, so the kernel minimises -cor (fp32) and maps to F_cor only on output.
 enum Objective { kObjChi2 = 0, kObjCor = 1 };
+// Third evaluation kind, chosen per block at run time under kObjChi2: the amplitude slope is fixed at zero (the caller's a1
+// box is [0, 0]; "c5 ... can be ignored when amplitude change is small with data length below 10 seconds"),
+// so A(t) = a0 and the amplitude FFMA2 drops out: 6 instead of 7 FP32 operations per sample-evaluation.
+constexpr int kEvalChi2Const = 2;
 
 struct BlockParams {
     const float* x;               // [B][N] fp32 samples, or null when the samples are quantised:
@@ -160,7 +164,9 @@ __device__ __forceinline__ void eval_chunk(const float4 xv, const float4 wv, con
             if (OBJ == kObjCor) {
                 acc[q] = fma2(cs, x2, acc[q]);                     // Eq. 5-6: sum x cos(phi); a padded sample has x = 0
             } else {
-                f32x2 A = fma2(na1[q], t2, na0[q]);
+                f32x2 A;
+                if (OBJ == kEvalChi2Const) A = na0[q];             // constant amplitude (a1 = 0)
+                else A = fma2(na1[q], t2, na0[q]);
                 if (MASKED && j >= n_left) A = pack2(0.0f, 0.0f);  // padded sample: residual 0 - 0 * c
                 const f32x2 r = fma2(A, cs, x2);
                 acc[q] = fma2(r, r, acc[q]);
@@ -505,6 +511,7 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                 const double l = p.lo[blk * D + tid], h = p.hi[blk * D + tid];
                 lo_s[tid] = l; hi_s[tid] = h;
                 base[tid] = 0.5 * (l + h);
+                if (tid == 1) base[7] = (l == 0.0 && h == 0.0) ? 1.0 : 0.0;     // amplitude slope fixed at zero
             }
         } else {
             if (tid < D) {   // mid-range of the given population
@@ -512,6 +519,7 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                 float mn = pp[0], mx = pp[0];
                 for (int i = 1; i < p.NP; ++i) { const float v = pp[(size_t)i * D]; mn = fminf(mn, v); mx = fmaxf(mx, v); }
                 base[tid] = 0.5 * ((double)mn + (double)mx);
+                if (tid == 1) base[7] = (mn == 0.0f && mx == 0.0f) ? 1.0 : 0.0;
             }
         }
         __syncthreads();
@@ -530,6 +538,18 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                 else wref[n] = (float)(kTwoPi * u);
             }
         }
+
+        // one evaluation pass of the table `cand`; the constant-amplitude loop when this block's a1 is fixed at zero
+        const bool a1z = (OBJ == kObjChi2) && base[7] != 0.0;
+        auto evaluate = [&]() {
+            if (STREAM) {
+                if (a1z) eval_population_streamed<C, D, (OBJ == kObjChi2 ? kEvalChi2Const : OBJ)>(p, st, cand, part, tid, warp, lane);
+                else eval_population_streamed<C, D, OBJ>(p, st, cand, part, tid, warp, lane);
+            } else {
+                if (a1z) eval_population<C, D, (OBJ == kObjChi2 ? kEvalChi2Const : OBJ)>(p, sl, xs, wref, cand, part, warp, lane);
+                else eval_population<C, D, OBJ>(p, sl, xs, wref, cand, part, warp, lane);
+            }
+        };
 
         // ---- a1: generation 0 ----
         const uint32_t bidx = (MODE == kModeFit) ? (p.block_index ? p.block_index[blk] : (uint32_t)blk) : 0u;
@@ -550,12 +570,12 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
             fence_proxy_async_global();      // workspace rows written above are read by the bulk copies below
             __syncthreads();
             if (tid == 0) stream_begin_block(p, st, xrow, wrow, (MODE == kModeFit) ? (uint32_t)p.G + 1u : 1u);
-            eval_population_streamed<C, D, OBJ>(p, st, cand, part, tid, warp, lane);
+            evaluate();
         } else {
             if (p.use_bulk) mbar_wait(bar, parity);
             parity ^= 1u;
             __syncthreads();
-            eval_population<C, D, OBJ>(p, sl, xs, wref, cand, part, warp, lane);
+            evaluate();
         }
         __syncthreads();
         combine_begin();
@@ -602,8 +622,7 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                     write_cand<D>(cand, i, th, base);
                 }
                 __syncthreads();
-                if (STREAM) eval_population_streamed<C, D, OBJ>(p, st, cand, part, tid, warp, lane);
-                else eval_population<C, D, OBJ>(p, sl, xs, wref, cand, part, warp, lane);
+                evaluate();
                 __syncthreads();
                 combine_begin();
                 // ---- a6: greedy selection, accept on <= ----

@@ -255,3 +255,39 @@ def test_cor_diverges_with_a_free_amplitude(pt):
     g, o = _both(pt, wl, wl.lo, wl.hi, NP=40, G=200, F=0.5, CR=0.9, seed=5, strategy=1, objective=1)
     for res in (g, o):
         assert np.all(np.abs(res["best"][:, 0] - wl.hi[:, 0]) <= 1e-3 * (wl.hi[:, 0] - wl.lo[:, 0]))
+
+
+# ----------------------------------------------------------------------------------------------
+# constant amplitude under the chi^2 objective: a1 fixed at zero takes the shorter evaluation loop
+# ----------------------------------------------------------------------------------------------
+def test_fixed_zero_amplitude_slope(pt):
+    """The caller's a1 box is [0, 0]: the kernel drops the amplitude FFMA2 (a per-block run-time choice).  Objective values
+    and fits against the oracle, resident / streamed / cluster paths, and blocks with and without the fixed slope mixed in
+    one launch."""
+    wl = W.config0(cases=range(6), a1_zero=True)
+    lo, hi = wl.lo.copy(), wl.hi.copy()
+    lo[:, 1] = hi[:, 1] = 0.0
+    lo[3:, 1], hi[3:, 1] = -0.05, 0.05                           # blocks 3..5 keep a free slope
+    rng = np.random.default_rng(0)
+    pop = (lo[:, None, :] + (hi - lo)[:, None, :] * rng.uniform(0, 1, size=(6, 64, 5))).astype(np.float32)
+    ref = oracle.fitness(wl.x, wl.fs, pop)
+    got = pt.pt_fitness(_cuda(wl.x), wl.fs, _cuda(pop)).cpu().numpy()
+    assert np.all(pop[:3, :, 1] == 0) and np.any(pop[3:, :, 1] != 0)
+    assert np.max(np.abs(got - ref) / ref) < REL_TOL
+    for K in (1, 4):
+        with _forced_cluster(K):
+            g, o = _both(pt, wl, lo, hi, NP=60, G=400, F=0.5, CR=0.9, seed=12, strategy=1)
+        assert np.all(g["best"][:3, 1] == 0.0)
+        assert np.max(np.abs(_wrap(g["best"][:, 2] - o["best"][:, 2]))) < PHI0_TOL
+        assert np.max(np.abs(g["best"][:, 3] - o["best"][:, 3])) < F_TOL
+        assert np.max(np.abs(g["best_rss"] - o["best_rss"]) / o["best_rss"]) < REL_TOL
+    # streamed blocks, ragged tail
+    with _forced_cluster(1):
+        ws = W.single_tone_blocks(range(2), 65536 + 132, 65536.0, config=4, f_range=(50.0, 200.0), a1_zero=True)
+        pop = np.repeat(ws.truth[:, None, :], 16, axis=1)
+        pop[:, :, 3] += np.linspace(-0.2, 0.2, 16)[None, :]
+        pop = pop.astype(np.float32)
+        assert np.all(pop[:, :, 1] == 0)
+        ref = oracle.fitness(ws.x, ws.fs, pop)
+        got = pt.pt_fitness(_cuda(ws.x), ws.fs, _cuda(pop)).cpu().numpy()
+        assert np.max(np.abs(got - ref) / ref) < REL_TOL
