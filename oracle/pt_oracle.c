@@ -25,7 +25,11 @@
  * numbers and index logic are exact integer arithmetic (Philox4x32-10).
  *
  * Pins (tests/test_oracle_*.py): Philox known answers; exhaustive index-draw checks; closed-form
- * fitness values; brute-force grid; Levenberg-Marquardt agreement; Appendix A of the paper.
+ * fitness values; brute-force grid; Levenberg-Marquardt agreement; Appendix A of the paper;
+ * for the mutation strategies the invariants of their definitions on every trial vector and the
+ * Levenberg-Marquardt optimum (the paper prints no values: it does not define them, reading R21);
+ * for Eq. 5 the limit the paper prints (0.31830988618), closed forms on whole cycles and the
+ * least-squares phase; for the sample unpacking hand-decoded bytes and numpy's integer views.
  * Parity unpinned, by design: fdot / fddot / a1 where the data cannot observe them.
  *
  * OpenMP is used only to spread independent blocks (or independent candidates of one
