@@ -273,6 +273,8 @@ def main():
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--ref-generations", type=int, default=100)
     ap.add_argument("--strategy", type=int, default=0, help="mutation strategy 1..6 (Table 4); 0 = the workload's own (DE/rand/1)")
+    ap.add_argument("--quant", type=int, default=0, choices=[0, 1, 2, 4, 8, 16],
+                    help="feed packed samples of this many bits (Table 3 formats, pt_fit_blocks_q / pt_track_host_q)")
     ap.add_argument("--fix-a1", action="store_true", help="fix the amplitude slope at zero (a1 box [0, 0], PAPER.md:139)")
     ap.add_argument("--objective", default="chi2", choices=["chi2", "cor"], help="Eq. 4 (default) or Eq. 5-6")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -314,7 +316,15 @@ def main():
                          seed=1 + rank, t0=wl.t0, strategy=wl.de["strategy"], objective=wl.de["objective"])
     plan = pt.pt_fit_blocks_plan(wl.B, wl.N, cfg)
     m_int = [max(1, int(round(tc / wl.T))) for tc in (1.0, 10.0, 60.0)]
-    x_h = torch.from_numpy(wl.x).pin_memory()
+    quant, qkw = None, {}
+    if args.quant:      # the receiver's recording format (Table 3): packed samples, unpacked in-kernel while staging
+        from paper_1906_10598_b200 import workloads as W
+        xq, qd = W.quantise(wl.x, args.quant)
+        quant = pt.make_quant(qd["bits"], qd["is_signed"], qd["scale"], qd["offset"])
+        qkw = dict(quant=quant, N=wl.N)
+        x_h = torch.from_numpy(xq).pin_memory()
+    else:
+        x_h = torch.from_numpy(wl.x).pin_memory()
     lo_h = torch.from_numpy(wl.lo).pin_memory()
     hi_h = torch.from_numpy(wl.hi).pin_memory()
     x, lo, hi = x_h.to(dev), lo_h.to(dev), hi_h.to(dev)
@@ -324,7 +334,7 @@ def main():
     def step(ev=None):
         if ev:
             ev[0].record()
-        r = pt.pt_fit_blocks(x, wl.fs, lo, hi, cfg)
+        r = pt.pt_fit_blocks(x, wl.fs, lo, hi, cfg, **qkw)
         if ev:
             ev[1].record()
         prod = pt.pt_doppler_products(r["best"], wl.T, 0.0, m_int)
@@ -365,19 +375,19 @@ def main():
     # ---- end to end through the C ABI with HOST buffers (H2D + fit + products + D2H inside the timed region) ----
     e2e = None
     if not args.no_e2e:
-        pt.pt_track_host(x_h, wl.fs, lo_h, hi_h, cfg, 0.0, m_int)          # warm-up
+        pt.pt_track_host(x_h, wl.fs, lo_h, hi_h, cfg, 0.0, m_int, **qkw)          # warm-up
         barrier()
         t0 = time.perf_counter()
         n_e2e = max(1, min(args.steps, 2))
         for _ in range(n_e2e):
-            out = pt.pt_track_host(x_h, wl.fs, lo_h, hi_h, cfg, 0.0, m_int)
+            out = pt.pt_track_host(x_h, wl.fs, lo_h, hi_h, cfg, 0.0, m_int, **qkw)
         barrier()
         e2e_s = (time.perf_counter() - t0) / n_e2e
         if dist is not None:
             tt = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
             e2e_s = float(tt.item())
-        h2d = x_h.numel() * 4 + lo_h.numel() * 8 + hi_h.numel() * 8
+        h2d = x_h.numel() * x_h.element_size() + lo_h.numel() * 8 + hi_h.numel() * 8
         d2h = sum(v.numel() * v.element_size() for k, v in out.items() if k != "intervals") + \
             sum(v.numel() * 8 for v in out["intervals"])
         e2e = {"value": units * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
@@ -411,6 +421,8 @@ def main():
     # initial ranges of every block, and the continuity check of the fitted track (no block of a clean track is re-searched)
     extras = {}
     try:
+        if quant is not None:
+            raise RuntimeError("skipped: acquisition and continuity check take fp32 samples")
         M = 1 << int(np.floor(np.log2(max(8, min(4096, wl.N // 2)))))
         acq = pt.make_acq_config(M=M, spacing=(wl.N - M) // 2, f_rel=0.0, f_bins=2.0, fdot_bins=2.0, a_rel=0.2)
         retry = pt.make_retry_config(phi_tol=1.5, F_tol=2.0)
@@ -442,6 +454,8 @@ def main():
             # columns, prefix scan) and one kernel per integration interval
             "gpu_launches": args.steps * ((2 if plan.get("tail_cluster") else 1) + 2 + len([m for m in m_int if wl.B // m > 0])),
             "peaks_file": _peaks().get("when")}
+    if quant is not None:
+        line["config"]["samples"] = "%d-bit packed (Table 3), unpacked in-kernel" % args.quant
     line.update(extras)
     if e2e is not None:
         line["e2e"] = e2e
