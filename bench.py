@@ -402,7 +402,7 @@ def main():
     sm_mhz = clocks.get("sm_mhz") or SM_MAX_MHZ
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": XU_PEAK / 1e12, "unit": "T sample-evals/s (1 MUFU cosine each)",
                 "frac": achieved / XU_PEAK,
-                "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.workload) if not wl.de["objective"] else None,
+                "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.workload) if not (wl.de["objective"] or args.quant) else None,
                 "kernel": "pt_block_kernel<C=%d,D=%d,fit,%s>" % (plan["cands_per_thread"], wl.de["D"],
                                                                 "cor" if wl.de["objective"] else "chi2"),
                 "kernel_ms": fit_ms, "peak_source": "derived: 148 SMs x 16 MUFU lanes x 1965 MHz (DESIGN.md); "
