@@ -35,8 +35,30 @@ SM_COUNT = 148
 XU_LANES_PER_SM = 16            # MUFU lanes per SM (4 per sub-partition): one cosine per sample-evaluation
 SM_MAX_MHZ = 1965.0
 XU_PEAK = SM_COUNT * XU_LANES_PER_SM * SM_MAX_MHZ * 1e6     # 4.65e12 sample-evaluations/s, DESIGN.md "Roofline"
-# dram__bytes_read.sum + dram__bytes_write.sum of one pt_block_kernel launch, from the ncu capture in profiles/
-TRAFFIC_BYTES_PER_LAUNCH = {"config2": 2.44e8}     # profiles/r1e_bench_launches.md (main + tail launch of one step, reads)
+# dram__bytes_read.sum + dram__bytes_write.sum of the DE-kernel launches of one step, from an `ncu --set full` capture of the
+# same command (profile file named beside the number); reported as roofline.traffic_ncu, never as a live measurement
+NCU_TRAFFIC = {"config2": {"bytes": 2.44e8, "source": "profiles/r1e_bench_launches.md (main + tail launch of one step)"}}
+
+
+def peak_probe(kind: int) -> float:
+    """Measured ALU stream rate of the device (bench-only library libpt_probe.so): kind 0 FFMA, kind 1 MUFU.COS."""
+    import ctypes as C
+    from paper_1906_10598_b200 import build as _b
+    lib = C.CDLL(_b.build_probe())
+    lib.pt_bench_peak_probe.argtypes = [C.c_int32, C.c_void_p]
+    lib.pt_bench_peak_probe.restype = C.c_int32
+    v = C.c_double(0.0)
+    rc = lib.pt_bench_peak_probe(int(kind), C.byref(v))
+    if rc != 0:
+        raise RuntimeError("pt_bench_peak_probe failed (%d)" % rc)
+    return float(v.value)
+
+
+def algorithmic_traffic(wl, quant_bits: int = 0) -> float:
+    """Bytes one step must move through HBM: every sample once, the boxes, and the per-block outputs."""
+    D = wl.de["D"]
+    samples = wl.B * wl.N * (quant_bits / 8.0 if quant_bits else 4.0)
+    return float(samples + wl.B * (2 * D * 8 + D * 8 + 4 + 4))
 
 
 def _peaks():
@@ -402,7 +424,10 @@ def main():
     sm_mhz = clocks.get("sm_mhz") or SM_MAX_MHZ
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": XU_PEAK / 1e12, "unit": "T sample-evals/s (1 MUFU cosine each)",
                 "frac": achieved / XU_PEAK,
-                "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.workload) if not (wl.de["objective"] or args.quant) else None,
+                # algorithmic bytes of one step, computed from the workload; the ncu-measured DRAM bytes of the same command
+                # (a committed profile, not this run) ride along as traffic_ncu
+                "traffic": algorithmic_traffic(wl, args.quant),
+                "traffic_ncu": NCU_TRAFFIC.get(args.workload) if not (wl.de["objective"] or args.quant or args.strategy) else None,
                 "kernel": "pt_block_kernel<C=%d,D=%d,fit,%s>" % (plan["cands_per_thread"], wl.de["D"],
                                                                 "cor" if wl.de["objective"] else "chi2"),
                 "kernel_ms": fit_ms, "peak_source": "derived: 148 SMs x 16 MUFU lanes x 1965 MHz (DESIGN.md); "
@@ -412,8 +437,8 @@ def main():
                 "fp32_flops_achieved_tflops": achieved * ((10 if wl.de["D"] == 5 else 12) - (4 if wl.de["objective"] else
                                                             (2 if wl.meta.get("fix_a1") else 0))) / 1e12}
     try:
-        roofline["measured_mufu_peak"] = pt.pt_peak_probe(1) / 1e12
-        roofline["measured_ffma_peak_tflops"] = 2 * pt.pt_peak_probe(0) / 1e12
+        roofline["measured_mufu_peak"] = peak_probe(1) / 1e12
+        roofline["measured_ffma_peak_tflops"] = 2 * peak_probe(0) / 1e12
     except Exception as exc:  # diagnostics only
         roofline["probe_error"] = str(exc)
 

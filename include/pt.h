@@ -16,8 +16,10 @@
  *     (the Python binding allocates them with torch).  Layouts are dense row-major.  Inputs are never
  *     modified.  The library keeps no device memory between calls; scratch is passed in by the caller and
  *     sized by the *_workspace_bytes query.
- *   - Device entry points are asynchronous on the given stream and never synchronise the device.
- *     The *_host entry point is synchronous and owns its temporary device memory.
+ *   - Device entry points are asynchronous on the given stream and never synchronise the device or the stream.
+ *     The *_host entry points are synchronous and own their temporary device memory.
+ *   - One process may drive several devices from several host threads: per-device state inside the library is keyed by
+ *     the CUDA device current at the call and guarded by a mutex.
  *   - The stream argument is a cudaStream_t passed as void* (NULL = the legacy default stream).
  *   - There is no CPU fallback: without a CUDA device every compute call returns PT_ERR_CUDA.
  */
@@ -39,7 +41,8 @@ extern "C" {
 
 typedef enum {
     PT_OK = 0,
-    PT_ERR_INVALID_ARG = -1, /* null pointer, N odd or < 8, D not 5/6, NP < 4, lo > hi, fs <= 0, F or CR out of range */
+    PT_ERR_INVALID_ARG = -1, /* null pointer, N odd or < 8, D not 5/6, NP < 4, fs <= 0, F or CR out of range; lo > hi in
+                                HOST boxes (*_host entries; device boxes: status bit4 of the block)            */
     PT_ERR_UNSUPPORTED = -2, /* NP or N beyond the compiled limits, workspace too small                               */
     PT_ERR_CUDA = -3         /* a CUDA call failed; see pt_last_error_string()                                        */
 } pt_status;
@@ -104,6 +107,14 @@ PT_API int32_t pt_fitness(const float* x, int64_t B, int32_t N, double fs, doubl
                    int32_t D, float* fitness, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * pt_objective -- like pt_fitness for either objective: objective = PT_OBJECTIVE_CHI2 writes Eq. 4,
+ * PT_OBJECTIVE_COR writes F_cor - 1/pi of Eq. 5-6 (see pt_objective_kind).  Same arguments otherwise.
+ */
+PT_API int32_t pt_objective(const float* x, int64_t B, int32_t N, double fs, double t0, const float* pop, int32_t NP,
+                     int32_t D, int32_t objective, float* fitness, void* workspace, size_t workspace_bytes,
+                     void* stream);
+
+/*
  * pt_fit_blocks -- Differential Evolution fit of every block (PAPER.md:39-43 Fig. 1, :203-224 Table 4):
  * NP members drawn uniformly in the box [lo, hi], then `generations` synchronous
  * generations of mutation by cfg->strategy (default DE/rand/1: v = x_r1 + F (x_r2 - x_r3)), binomial crossover
@@ -117,21 +128,19 @@ PT_API int32_t pt_fitness(const float* x, int64_t B, int32_t N, double fs, doubl
  * best         [B][D]     fp64 out: member with the smallest RSS (lowest index on ties)
  * best_rss     [B]        fp32 out: its RSS (the "RSS" column of the paper's output record);
  *                                   F_cor - 1/pi for PT_OBJECTIVE_COR
- * status       [B]        u32 out: bit0 = best lies within 1e-6 (hi-lo) of a box face;
- *                                  bit1 = population not collapsed (max RSS - min RSS > 1e-3 min RSS; for the
- *                                         correlation objective the same rule on F_cor - 1/pi)
+ * status       [B]        u32 out: bit0 (1) = best lies within 1e-6 (hi-lo) of a box face;
+ *                                  bit1 (2) = population not collapsed (max RSS - min RSS > 1e-3 min RSS; for the
+ *                                         correlation objective the same rule on F_cor - 1/pi);
+ *                                  bit2 (4) = abandoned by pt_refit_doubtful;
+ *                                  bit3 (8) = the best member's objective is not finite (a NaN or Inf sample in the
+ *                                         block): the block's outputs are meaningless, the other blocks are unaffected;
+ *                                  bit4 (16) = the block's box has lo > hi (or a NaN) in some coordinate.  The device
+ *                                         entry points are asynchronous and cannot return PT_ERR_INVALID_ARG for the
+ *                                         contents of device arrays; pt_track_host checks its host boxes and does.
  * final_pop    [B][NP][D] fp32 out, optional (NULL): final population rounded to fp32
  * final_fit    [B][NP]    fp32 out, optional (NULL)
  * workspace               >= pt_fit_blocks_workspace_bytes(B, N, cfg) bytes of device scratch (may be NULL if 0)
  */
-/*
- * pt_objective -- like pt_fitness for either objective: objective = PT_OBJECTIVE_CHI2 writes Eq. 4,
- * PT_OBJECTIVE_COR writes F_cor - 1/pi of Eq. 5-6 (see pt_objective_kind).  Same arguments otherwise.
- */
-PT_API int32_t pt_objective(const float* x, int64_t B, int32_t N, double fs, double t0, const float* pop, int32_t NP,
-                     int32_t D, int32_t objective, float* fitness, void* workspace, size_t workspace_bytes,
-                     void* stream);
-
 PT_API size_t pt_fit_blocks_workspace_bytes(int64_t B, int32_t N, const pt_de_config* cfg /*[host]*/);
 PT_API int32_t pt_fit_blocks(const float* x, int64_t B, int32_t N, double fs, const double* lo, const double* hi,
                       const uint32_t* block_index, const pt_de_config* cfg /*[host]*/, double* best,
@@ -221,7 +230,9 @@ PT_API int32_t pt_acquire(const float* x, int64_t B, int32_t N, double fs, int32
  * lo, hi, best, best_rss, status [B]... are those of the preceding pt_fit_blocks call and are updated in place;
  * attempts [B] int32 device out: re-searches each block took (set to 0 first).
  * workspace: >= pt_refit_doubtful_workspace_bytes(B, N, cfg) device bytes, 16-byte aligned.
- * The call synchronises `stream` once per attempt (the list of doubtful blocks is compacted on the host).
+ * Asynchronous like every device entry point: the list of doubtful blocks and its length stay on the device (ordered
+ * compaction kernel), every attempt is enqueued unconditionally and its kernels do nothing once no block is doubtful.  The
+ * re-fit launch therefore has the geometry of B single-CTA blocks; CTAs without a doubtful block exit at once.
  */
 typedef struct {
     double phi_tol;       /* rad                                                              */
@@ -306,14 +317,6 @@ PT_API int32_t pt_de_draws(const uint32_t* query, int64_t Q, int32_t NP, int32_t
  */
 PT_API int32_t pt_init_population(const double* lo, const double* hi, const uint32_t* block_index, int64_t B, int32_t NP,
                            int32_t D, uint64_t seed, double* pop0, void* stream);
-
-/*
- * pt_peak_probe -- measured ALU peaks of the device, for the roofline denominators bench.py reports.
- * kind 0: dependent-free FFMA stream; kind 1: MUFU.COS stream; kind 2: the 7 FP32 + 1 MUFU mix of one
- * sample-evaluation.  Writes operations per second (fp32 lane-operations of the probed kind) to *ops_per_s [host].
- * Synchronous.
- */
-PT_API int32_t pt_peak_probe(int32_t kind, double* ops_per_s /*[host]*/);
 
 /* Launch geometry the library would use for pt_fit_blocks (for reporting): out[0] = grid, out[1] = threads per CTA,
  * out[2] = dynamic shared memory bytes, out[3] = 1 if the block's samples stay resident in shared memory, 0 if streamed,

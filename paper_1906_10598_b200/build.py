@@ -14,7 +14,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpt.so")
 STAMP = os.path.join(HERE, ".libpt.stamp")
-SOURCES = ["pt_api.cu", "pt_doppler.cu", "pt_probe.cu", "pt_acquire.cu", "pt_retry.cu"]
+SOURCES = ["pt_api.cu", "pt_doppler.cu", "pt_acquire.cu", "pt_retry.cu"]
+# bench-only micro-benchmarks (measured FFMA / MUFU stream rates): their own library, not part of the product ABI
+PROBE_LIB = os.path.join(HERE, "libpt_probe.so")
+PROBE_STAMP = os.path.join(HERE, ".libpt_probe.stamp")
+PROBE_SOURCES = ["pt_probe.cu"]
 NVCC_FLAGS = [
     "-O3",
     "-std=c++17",
@@ -43,24 +47,34 @@ def _fingerprint() -> str:
     return h.hexdigest()
 
 
-def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
-    """Compile csrc/*.cu into libpt.so; skipped when sources and flags are unchanged."""
+def _build(lib: str, stamp: str, sources, force: bool, verbose: bool, extra_flags) -> str:
     fp = _fingerprint()
-    if not force and not extra_flags and os.path.exists(LIB) and os.path.exists(STAMP):
-        with open(STAMP) as fh:
+    if not force and not extra_flags and os.path.exists(lib) and os.path.exists(stamp):
+        with open(stamp) as fh:
             if fh.read().strip() == fp:
-                return LIB
-    tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [_nvcc()] + NVCC_FLAGS + list(extra_flags) + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
+                return lib
+    tmp = lib + ".tmp.%d" % os.getpid()
+    cmd = [_nvcc()] + NVCC_FLAGS + list(extra_flags) + ["-o", tmp] + [os.path.join(CSRC, s) for s in sources]
     if verbose:
         print(" ".join(cmd), file=sys.stderr)
     subprocess.run(cmd, check=True)
-    os.replace(tmp, LIB)
-    with open(STAMP, "w") as fh:
+    os.replace(tmp, lib)
+    with open(stamp, "w") as fh:
         fh.write(fp)
-    return LIB
+    return lib
+
+
+def build(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
+    """Compile csrc/*.cu into libpt.so; a no-op when sources and flags are unchanged (fingerprint stamp)."""
+    return _build(LIB, STAMP, SOURCES, force, verbose, extra_flags)
+
+
+def build_probe(force: bool = False, verbose: bool = False) -> str:
+    """Compile the bench-only peak probes into libpt_probe.so."""
+    return _build(PROBE_LIB, PROBE_STAMP, PROBE_SOURCES, force, verbose, ())
 
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose=True,
                 extra_flags=["-Xptxas", "-v"] if "--ptxas-v" in sys.argv else ()))
+    print(build_probe(force="--force" in sys.argv, verbose=True))

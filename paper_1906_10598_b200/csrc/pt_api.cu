@@ -5,6 +5,7 @@
 #include <cstdlib>
 #include <cmath>
 #include <algorithm>
+#include <mutex>
 #include <vector>
 
 #include "../../include/pt.h"
@@ -38,17 +39,27 @@ struct Plan {
     int K, NpadS;           // cluster path: CTAs per block, padded samples of the largest slice (K = 1: Npad)
 };
 
-static int device_info(int* sms, int* smem_optin) {
-    static int cached_dev = -1, c_sms = 0, c_smem = 0;
+// Per-device facts and per-device launch attributes, keyed by the CUDA device ordinal and guarded by one mutex: a process may
+// drive several devices, from several host threads.
+constexpr int kMaxDevices = 64;
+static std::mutex g_dev_mutex;
+struct DeviceFacts { int known, sms, smem_optin; };
+static DeviceFacts g_dev[kMaxDevices];
+
+static int device_info(int* sms, int* smem_optin, int* dev_out = nullptr) {
     int dev = 0;
     if (check_cuda(cudaGetDevice(&dev), "cudaGetDevice")) return 1;
-    if (dev != cached_dev) {
-        if (check_cuda(cudaDeviceGetAttribute(&c_sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute")) return 1;
-        if (check_cuda(cudaDeviceGetAttribute(&c_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev), "cudaDeviceGetAttribute")) return 1;
-        cached_dev = dev;
+    if (dev < 0 || dev >= kMaxDevices) { set_error("device ordinal %d beyond the compiled limit %d", dev, kMaxDevices); return 1; }
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    DeviceFacts& f = g_dev[dev];
+    if (!f.known) {
+        if (check_cuda(cudaDeviceGetAttribute(&f.sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute")) return 1;
+        if (check_cuda(cudaDeviceGetAttribute(&f.smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev), "cudaDeviceGetAttribute")) return 1;
+        f.known = 1;
     }
-    *sms = c_sms;
-    *smem_optin = c_smem;
+    *sms = f.sms;
+    *smem_optin = f.smem_optin;
+    if (dev_out) *dev_out = dev;
     return 0;
 }
 
@@ -140,7 +151,7 @@ static int force_cluster() {
 }
 
 // plan with the current device's limits, or B200's when no device is present (the query entry points)
-static int plan_for(long long B, int N, int NP, int D, Plan* pl, bool need_device) {
+static int plan_for(long long B, int N, int NP, int D, Plan* pl, bool need_device, int force_K = 0) {
     int sms = 148, smem_optin = 232448;
     int dev_count = 0;
     if (cudaGetDeviceCount(&dev_count) == cudaSuccess && dev_count > 0) {
@@ -149,7 +160,7 @@ static int plan_for(long long B, int N, int NP, int D, Plan* pl, bool need_devic
         (void)cudaGetLastError();
         if (need_device) { set_error("no CUDA device"); return PT_ERR_CUDA; }
     }
-    if (make_plan(B, N, NP, D, sms, smem_optin, force_cluster(), pl)) {
+    if (make_plan(B, N, NP, D, sms, smem_optin, force_K > 0 ? force_K : force_cluster(), pl)) {
         set_error("N = %d with NP = %d: population tables alone exceed shared memory", N, NP);
         return PT_ERR_UNSUPPORTED;
     }
@@ -169,13 +180,19 @@ static void cluster_launch_config(const Plan& pl, int grid, cudaStream_t st, cud
 
 template <int C, int D, int MODE, bool STREAM, int OBJ>
 static int configure_smem(const Plan& pl) {
-    static int configured_smem = -1;
-    if (pl.smem > configured_smem) {
+    // cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute of the kernel: remember the largest value set on
+    // each device (one table per template instantiation)
+    static int configured_smem[kMaxDevices];
+    int dev = 0;
+    if (check_cuda(cudaGetDevice(&dev), "cudaGetDevice")) return PT_ERR_CUDA;
+    if (dev < 0 || dev >= kMaxDevices) { set_error("device ordinal %d beyond the compiled limit %d", dev, kMaxDevices); return PT_ERR_CUDA; }
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    if (pl.smem > configured_smem[dev]) {
         if (check_cuda(cudaFuncSetAttribute(pt_block_kernel<C, D, MODE, STREAM, OBJ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             pl.smem),
                        "cudaFuncSetAttribute"))
             return PT_ERR_CUDA;
-        configured_smem = pl.smem;
+        configured_smem[dev] = pl.smem;
     }
     return PT_OK;
 }
@@ -351,12 +368,6 @@ __global__ void unpack_samples_kernel(const unsigned char* __restrict__ xq, long
     }
 }
 
-__global__ void check_box_kernel(const double* __restrict__ lo, const double* __restrict__ hi, long long n, int* bad) {
-    const long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (k >= n) return;
-    if (!(lo[k] <= hi[k])) atomicExch(bad, 1);
-}
-
 }  // namespace pt
 
 using namespace pt;
@@ -427,8 +438,10 @@ static int32_t fit_blocks_impl(const float* x, const unsigned char* xq, const pt
                                int32_t N, double fs, const double* lo, const double* hi, const uint32_t* block_index,
                                const pt_de_config* cfg, double* best, float* best_rss, uint32_t* status, float* final_pop,
                                float* final_fit, void* workspace, size_t workspace_bytes, void* stream,
-                               const uint32_t* sel = nullptr) {
-    // sel != null: B work items, item j is data block sel[j] of the caller's arrays (pt_refit_doubtful)
+                               const uint32_t* sel = nullptr, const int* count = nullptr) {
+    // sel != null: work item j is data block sel[j] of the caller's arrays; count (device scalar) = how many items there are,
+    // at most B (pt_refit_doubtful: the number of doubtful blocks is known on the device only, so the launch geometry is that
+    // of B single-CTA blocks and CTAs without an item exit at once)
     if ((!x && !xq) || !lo || !hi || !best || !best_rss || !status) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
     int rc = check_cfg(cfg);
     if (rc) return rc;
@@ -441,10 +454,10 @@ static int32_t fit_blocks_impl(const float* x, const unsigned char* xq, const pt
         if (rc) return rc;
     }
     Plan pl;
-    rc = plan_for(B, N, cfg->NP, cfg->D, &pl, true);
+    rc = plan_for(B, N, cfg->NP, cfg->D, &pl, true, count ? 1 : 0);
     if (rc) return rc;
     p.x = x; p.xq = xq; p.row_bytes = row_bytes;
-    p.lo = lo; p.hi = hi; p.block_index = block_index; p.sel = sel;
+    p.lo = lo; p.hi = hi; p.block_index = block_index; p.sel = sel; p.count = count;
     p.best = best; p.best_rss = best_rss; p.status = status; p.final_pop = final_pop; p.final_fit = final_fit;
     p.B = B; p.N = N; p.Npad = pl.Npad; p.NP = cfg->NP; p.NPpad = pl.NPpad; p.G = cfg->generations;
     p.fs = fs; p.t0 = cfg->t0; p.F = cfg->F;
@@ -456,7 +469,7 @@ static int32_t fit_blocks_impl(const float* x, const unsigned char* xq, const pt
     rc = attach_workspace(&p, pl, workspace, workspace_bytes);
     if (rc) return rc;
     Plan tl;
-    const long long rem = plan_tail(B, N, cfg->NP, cfg->D, pl, &tl);
+    const long long rem = count ? 0 : plan_tail(B, N, cfg->NP, cfg->D, pl, &tl);
     if (rem == 0) return dispatch<kModeFit>(p, pl, cfg->D, cfg->objective, (cudaStream_t)stream);
     // full waves on single CTAs, then the last partial wave on clusters
     p.B = B - rem;
@@ -520,19 +533,27 @@ int32_t pt_acquire(const float* x, int64_t B, int32_t N, double fs, int32_t D, c
     return PT_OK;
 }
 
-static void refit_layout(int64_t B, size_t fit_ws, size_t* o_pb, size_t* o_tp, size_t* o_flags, size_t* o_list, size_t* o_fit,
-                         size_t* total) {
+static void refit_layout(int64_t B, size_t fit_ws, size_t* o_pb, size_t* o_tp, size_t* o_flags, size_t* o_list, size_t* o_cnt,
+                         size_t* o_fit, size_t* total) {
     size_t off = 0;
     auto take = [&off](size_t bytes) { size_t o = off; off += (bytes + 255) / 256 * 256; return o; };
     *o_pb = take((size_t)B * 10 * 8); *o_tp = take((size_t)B * 8); *o_flags = take((size_t)B * 4); *o_list = take((size_t)B * 4);
+    *o_cnt = take(sizeof(int));
     *o_fit = take(fit_ws);
     *total = off;
 }
 
+// workspace of the re-fit launches: the plan of B single-CTA blocks (see fit_blocks_impl, count != null)
+static size_t refit_fit_workspace_bytes(int64_t B, int32_t N, const pt_de_config* cfg) {
+    Plan pl;
+    if (!cfg || check_common(B, N, 1.0, cfg->NP, cfg->D) || plan_for(B, N, cfg->NP, cfg->D, &pl, false, 1)) return 0;
+    return pl.ws_bytes;
+}
+
 size_t pt_refit_doubtful_workspace_bytes(int64_t B, int32_t N, const pt_de_config* cfg) {
     if (!cfg || B < 1) return 0;
-    size_t a, b, c, d, e, total;
-    refit_layout(B, pt_fit_blocks_workspace_bytes(B, N, cfg), &a, &b, &c, &d, &e, &total);
+    size_t a, b, c, d, e, f, total;
+    refit_layout(B, refit_fit_workspace_bytes(B, N, cfg), &a, &b, &c, &d, &e, &f, &total);
     return total;
 }
 
@@ -550,9 +571,9 @@ int32_t pt_refit_doubtful(const float* x, int64_t B, int32_t N, double fs, doubl
         set_error("invalid retry configuration");
         return PT_ERR_INVALID_ARG;
     }
-    const size_t fit_ws = pt_fit_blocks_workspace_bytes(B, N, cfg);
-    size_t o_pb, o_tp, o_flags, o_list, o_fit, total;
-    refit_layout(B, fit_ws, &o_pb, &o_tp, &o_flags, &o_list, &o_fit, &total);
+    const size_t fit_ws = refit_fit_workspace_bytes(B, N, cfg);
+    size_t o_pb, o_tp, o_flags, o_list, o_cnt, o_fit, total;
+    refit_layout(B, fit_ws, &o_pb, &o_tp, &o_flags, &o_list, &o_cnt, &o_fit, &total);
     if (!workspace || workspace_bytes < total) { set_error("pt_refit_doubtful needs %zu bytes of workspace, got %zu", total, workspace ? workspace_bytes : (size_t)0); return PT_ERR_UNSUPPORTED; }
     if (reinterpret_cast<uintptr_t>(workspace) % 16) { set_error("workspace must be 16-byte aligned"); return PT_ERR_INVALID_ARG; }
     int dev_count = 0;
@@ -562,41 +583,36 @@ int32_t pt_refit_doubtful(const float* x, int64_t B, int32_t N, double fs, doubl
     double* total_phase = reinterpret_cast<double*>(ws + o_tp);
     uint32_t* flags = reinterpret_cast<uint32_t*>(ws + o_flags);
     uint32_t* list = reinterpret_cast<uint32_t*>(ws + o_list);
+    int* count = reinterpret_cast<int*>(ws + o_cnt);
     cudaStream_t st = (cudaStream_t)stream;
     const int D = cfg->D;
     const double T = (double)N / fs;
     if (check_cuda(cudaMemsetAsync(attempts, 0, (size_t)B * sizeof(int32_t), st), "cudaMemsetAsync")) return PT_ERR_CUDA;
-    std::vector<uint32_t> h_flags((size_t)B), h_list;
+    // Eq. 8 residuals of the current solution -> flags of the doubtful blocks -> their ordered list and its length, all on the device
     auto flag_blocks = [&]() -> int {
         if (doppler_launch(best, B, D, T, 0.0, nullptr, 0, per_block, total_phase, nullptr, st)) return PT_ERR_CUDA;
         if (check_cuda(cudaGetLastError(), "doppler kernels launch")) return PT_ERR_CUDA;
         if (retry_flag_launch(per_block, B, retry->phi_tol, retry->F_tol, flags, st)) return PT_ERR_CUDA;
-        if (check_cuda(cudaMemcpyAsync(h_flags.data(), flags, (size_t)B * 4, cudaMemcpyDeviceToHost, st), "D2H flags")) return PT_ERR_CUDA;
-        if (check_cuda(cudaStreamSynchronize(st), "pt_refit_doubtful")) return PT_ERR_CUDA;
-        h_list.clear();
-        for (int64_t b = 0; b < B; ++b)
-            if (h_flags[(size_t)b]) h_list.push_back((uint32_t)b);
+        if (retry_compact_launch(flags, B, list, count, st)) return PT_ERR_CUDA;
         return PT_OK;
     };
+    // Every attempt is enqueued unconditionally: with no doubtful block left its kernels find *count == 0 and do nothing
+    // (a few launch latencies), which is what lets the call stay asynchronous.
     double g = 1.0;
     for (int a = 1; a <= retry->max_attempts; ++a, g *= retry->grow) {
         rc = flag_blocks();
         if (rc) return rc;
-        if (h_list.empty()) return PT_OK;
         if (retry_box_launch(flags, best, lo, hi, B, D, T, g, retry, st)) return PT_ERR_CUDA;
-        if (check_cuda(cudaMemcpyAsync(list, h_list.data(), h_list.size() * 4, cudaMemcpyHostToDevice, st), "H2D list")) return PT_ERR_CUDA;
         pt_de_config c = *cfg;
         c.seed = cfg->seed + (uint64_t)a * 0x9E3779B97F4A7C15ull;
-        rc = fit_blocks_impl(x, nullptr, nullptr, 0, (int64_t)h_list.size(), N, fs, lo, hi, block_index, &c, best, best_rss, status,
-                             nullptr, nullptr, fit_ws ? ws + o_fit : nullptr, fit_ws, st, list);
+        rc = fit_blocks_impl(x, nullptr, nullptr, 0, B, N, fs, lo, hi, block_index, &c, best, best_rss, status, nullptr, nullptr,
+                             fit_ws ? ws + o_fit : nullptr, fit_ws, st, list, count);
         if (rc) return rc;
-        if (retry_count_launch(list, (long long)h_list.size(), attempts, st)) return PT_ERR_CUDA;
-        // h_list is reused by the next attempt: the copy above must have been consumed
-        if (check_cuda(cudaStreamSynchronize(st), "pt_refit_doubtful")) return PT_ERR_CUDA;
+        if (retry_count_launch(list, count, B, attempts, st)) return PT_ERR_CUDA;
     }
     rc = flag_blocks();
     if (rc) return rc;
-    if (!h_list.empty() && retry->max_attempts > 0)
+    if (retry->max_attempts > 0)
         if (retry_abandon_launch(flags, B, status, st)) return PT_ERR_CUDA;
     return PT_OK;
 }
@@ -641,11 +657,6 @@ int32_t pt_init_population(const double* lo, const double* hi, const uint32_t* b
     else init_population_kernel<6><<<grid, thr, 0, (cudaStream_t)stream>>>(lo, hi, block_index, B, NP, k0, k1, pop0);
     if (check_cuda(cudaGetLastError(), "init_population_kernel launch")) return PT_ERR_CUDA;
     return PT_OK;
-}
-
-int32_t pt_peak_probe(int32_t kind, double* ops_per_s) {
-    if (!ops_per_s || kind < 0 || kind > 3) { set_error("invalid probe arguments"); return PT_ERR_INVALID_ARG; }
-    return peak_probe(kind, ops_per_s);
 }
 
 static int32_t track_host_impl(const float* x, const void* xq, const pt_quant* quant, int64_t row_bytes, int64_t B, int32_t N,

@@ -48,6 +48,8 @@ struct BlockParams {
     const double* hi;             // [B][D]  (fit)
     const uint32_t* block_index;  // [B] or null (fit)
     const uint32_t* sel;          // [B] or null: when given, work item j of [blk0, B) is data block sel[j] (re-search of a subset)
+    const int* count;             // device scalar or null: when given, only work items [blk0, blk0 + *count) exist (the length of
+                                  // sel, known on the device only: pt_refit_doubtful never synchronises)
     const float* pop_in;          // [B][NP][D] (fitness)
     float* fitness_out;           // [B][NP]    (fitness)
     double* best;                 // [B][D]
@@ -447,9 +449,12 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
     };
     // argmin of fit[0..NP) with the lowest index on ties, and the maximum; every lane of the calling warp gets them
     auto warp_argmin = [&](float& bv, int& bi, float& mx) {
+        // a NaN objective (a non-finite sample makes every member's sum NaN) compares false with everything: it is read
+        // as +inf, so that the index stays inside the population (all NaN -> member 0) and the block is flagged by status bit 3
         bv = INFINITY; mx = -INFINITY; bi = 0x7fffffff;
         for (int i = lane; i < p.NP; i += 32) {
-            const float v = fit[i];
+            float v = fit[i];
+            if (!(v == v)) v = INFINITY;
             if (v < bv || (v == bv && i < bi)) { bv = v; bi = i; }
             mx = fmaxf(mx, v);
         }
@@ -469,7 +474,8 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
         return (double)v;
     };
 
-    for (long long item = p.blk0 + first_blk; item < p.B; item += blk_stride) {
+    const long long item_end = p.count ? min(p.B, p.blk0 + (long long)*p.count) : p.B;
+    for (long long item = p.blk0 + first_blk; item < item_end; item += blk_stride) {
         const long long blk = p.sel ? (long long)p.sel[item] : item;
         const bool quantised = p.q.bits != 0;
         const float* xg = quantised ? nullptr : p.x + blk * (long long)p.N + n_lo;      // this CTA's slice of the block
@@ -513,6 +519,11 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                 base[tid] = 0.5 * (l + h);
                 if (tid == 1) base[7] = (l == 0.0 && h == 0.0) ? 1.0 : 0.0;     // amplitude slope fixed at zero
             }
+            if (tid == 32) {   // lo <= hi is the caller's contract (pt.h); an asynchronous call reports a violation in status bit 4
+                bool bad = false;
+                for (int j = 0; j < D; ++j) bad = bad || !(p.lo[blk * D + j] <= p.hi[blk * D + j]);
+                base[6] = bad ? 1.0 : 0.0;
+            }
         } else {
             if (tid < D) {   // mid-range of the given population
                 const float* pp = p.pop_in + blk * (long long)p.NP * D + tid;
@@ -521,6 +532,7 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                 base[tid] = 0.5 * ((double)mn + (double)mx);
                 if (tid == 1) base[7] = (mn == 0.0f && mx == 0.0f) ? 1.0 : 0.0;
             }
+            if (tid == 32) base[6] = 0.0;
         }
         __syncthreads();
 
@@ -652,14 +664,17 @@ __global__ void __launch_bounds__(512, 1) pt_block_kernel(const BlockParams p) {
                         const double w = hi_s[j] - lo_s[j];
                         if (w > 0.0 && (v - lo_s[j] <= 1e-6 * w || hi_s[j] - v <= 1e-6 * w)) st |= 1u;
                     }
+                    const float braw = fit[bi];                        // as evaluated (NaN stays NaN in the output)
                     if (OBJ == kObjCor) {
                         const double fb = reported(bv), fw = reported(mx);
                         if (fw - fb > 1e-3 * fb) st |= 2u;
-                        p.best_rss[blk] = (float)fb;
+                        p.best_rss[blk] = (float)reported(braw);
                     } else {
                         if (mx - bv > 1e-3f * bv) st |= 2u;
-                        p.best_rss[blk] = bv;
+                        p.best_rss[blk] = braw;
                     }
+                    if (!(fabsf(braw) <= 3.0e38f)) st |= 8u;           // objective of the best member is not finite
+                    if (base[6] != 0.0) st |= 16u;                     // the caller's box has lo > hi (or NaN) in some coordinate
                     p.status[blk] = st;
                 }
             }

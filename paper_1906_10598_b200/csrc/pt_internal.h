@@ -20,11 +20,9 @@ int acquire_launch(const float* x, long long B, int N, double fs, int D, const p
 int retry_flag_launch(const double* per_block, long long B, double phi_tol, double F_tol_hz, uint32_t* flags, cudaStream_t st);
 int retry_box_launch(const uint32_t* flags, const double* best, double* lo, double* hi, long long B, int D, double T, double g,
                      const pt_retry_config* rc, cudaStream_t st);
-int retry_count_launch(const uint32_t* sel, long long n, int32_t* attempts, cudaStream_t st);
+int retry_compact_launch(const uint32_t* flags, long long B, uint32_t* list, int* count, cudaStream_t st);
+int retry_count_launch(const uint32_t* sel, const int* n, long long B, int32_t* attempts, cudaStream_t st);
 int retry_abandon_launch(const uint32_t* flags, long long B, uint32_t* status, cudaStream_t st);
-
-// pt_probe.cu
-int peak_probe(int kind, double* ops_per_s);
 
 // pt_api.cu
 void set_error(const char* fmt, ...);

@@ -1,6 +1,6 @@
 // pt_retry.cu -- continuity check and run-time ranges of the re-search of doubtful blocks (section 3.1.1,
 // :226-248 section 3.1.3 Eq. 8, :252 section 3.1.4; reading R25).  Small fp64 kernels, one thread per block;
-// the host loop that strings them together with pt_fit_blocks is pt_refit_doubtful in pt_api.cu.
+// pt_refit_doubtful in pt_api.cu strings them together with the DE kernel, all on the caller's stream (no host round trip).
 #include <cmath>
 
 #include "pt_internal.h"
@@ -64,9 +64,49 @@ __global__ void retry_box_kernel(const uint32_t* __restrict__ flags, const doubl
     l[2] = -kPi; h[2] = kPi;
 }
 
-__global__ void retry_count_kernel(const uint32_t* __restrict__ sel, long long n, int32_t* __restrict__ attempts) {
+// Ordered compaction of the doubtful blocks: list[0 .. *count) = ascending indices b with flags[b] != 0.  One CTA walks the
+// flags in chunks of its size with a block-wide exclusive scan (B is a few 10^4: a few dozen trips), so the list is in the same
+// order a host loop would produce and no host round trip is needed.
+__global__ void __launch_bounds__(1024) retry_compact_kernel(const uint32_t* __restrict__ flags, long long B, uint32_t* __restrict__ list,
+                                                             int* __restrict__ count) {
+    __shared__ int warp_tot[32];
+    __shared__ int base;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) base = 0;
+    __syncthreads();
+    for (long long b0 = 0; b0 < B; b0 += blockDim.x) {
+        const long long b = b0 + tid;
+        const int f = (b < B && flags[b]) ? 1 : 0;
+        int incl = f;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, incl, off);
+            if (lane >= off) incl += v;
+        }
+        if (lane == 31) warp_tot[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            int t = warp_tot[lane];
+#pragma unroll
+            for (int off = 1; off < 32; off <<= 1) {
+                const int v = __shfl_up_sync(0xffffffffu, t, off);
+                if (lane >= off) t += v;
+            }
+            warp_tot[lane] = t;      // inclusive totals of the warps
+        }
+        __syncthreads();
+        const int before = base + (warp > 0 ? warp_tot[warp - 1] : 0) + incl - f;
+        if (f) list[before] = (uint32_t)b;
+        __syncthreads();
+        if (tid == 0) base += warp_tot[31];
+        __syncthreads();
+    }
+    if (tid == 0) *count = base;
+}
+
+__global__ void retry_count_kernel(const uint32_t* __restrict__ sel, const int* __restrict__ n, long long B, int32_t* __restrict__ attempts) {
     const long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (k < n) attempts[sel[k]] += 1;
+    if (k < B && k < *n) attempts[sel[k]] += 1;
 }
 
 __global__ void retry_abandon_kernel(const uint32_t* __restrict__ flags, long long B, uint32_t* __restrict__ status) {
@@ -88,8 +128,13 @@ int retry_box_launch(const uint32_t* flags, const double* best, double* lo, doub
     return check_cuda(cudaGetLastError(), "retry_box_kernel launch");
 }
 
-int retry_count_launch(const uint32_t* sel, long long n, int32_t* attempts, cudaStream_t st) {
-    retry_count_kernel<<<grid_for(n), 128, 0, st>>>(sel, n, attempts);
+int retry_compact_launch(const uint32_t* flags, long long B, uint32_t* list, int* count, cudaStream_t st) {
+    retry_compact_kernel<<<1, 1024, 0, st>>>(flags, B, list, count);
+    return check_cuda(cudaGetLastError(), "retry_compact_kernel launch");
+}
+
+int retry_count_launch(const uint32_t* sel, const int* n, long long B, int32_t* attempts, cudaStream_t st) {
+    retry_count_kernel<<<grid_for(B), 128, 0, st>>>(sel, n, B, attempts);
     return check_cuda(cudaGetLastError(), "retry_count_kernel launch");
 }
 

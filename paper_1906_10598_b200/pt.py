@@ -58,13 +58,11 @@ class RetryConfig(C.Structure):
 
 
 def lib():
-    """Load (building first if needed) the CUDA library.  Raises if that is impossible."""
+    """Load the CUDA library, (re)building it first when the sources changed.  Raises if that is impossible."""
     global _lib
     if _lib is not None:
         return _lib
-    path = _build.LIB
-    if not os.path.exists(path):
-        path = _build.build()
+    path = _build.build()        # a no-op when the fingerprint stamp matches; rebuilds a stale library after a source edit
     L = C.CDLL(path)
     p, i32, i64, f64, u64, sz = C.c_void_p, C.c_int32, C.c_int64, C.c_double, C.c_uint64, C.c_size_t
     L.pt_last_error_string.restype = C.c_char_p
@@ -104,8 +102,6 @@ def lib():
     L.pt_de_draws.restype = i32
     L.pt_init_population.argtypes = [p, p, p, i64, i32, i32, u64, p, p]
     L.pt_init_population.restype = i32
-    L.pt_peak_probe.argtypes = [i32, p]
-    L.pt_peak_probe.restype = i32
     _lib = L
     return L
 
@@ -372,9 +368,3 @@ def pt_init_population(lo: torch.Tensor, hi: torch.Tensor, NP: int, seed: int,
                                   out.data_ptr(), _stream())
     _check(rc, "pt_init_population")
     return out
-
-
-def pt_peak_probe(kind: int) -> float:
-    v = C.c_double(0.0)
-    _check(lib().pt_peak_probe(int(kind), C.byref(v)), "pt_peak_probe")
-    return float(v.value)

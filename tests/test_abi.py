@@ -128,3 +128,89 @@ def test_product_path_has_no_oracle_import():
                 with open(os.path.join(dirpath, f)) as fh:
                     text = fh.read()
                 assert "import oracle" not in text and "from oracle" not in text and "pt_oracle" not in text, f
+
+
+def test_lib_rebuilds_a_stale_library(monkeypatch):
+    """pt.lib() goes through build.build() every time (a no-op when the fingerprint stamp matches), so a source edit can never
+    leave tests running an old binary."""
+    from paper_1906_10598_b200 import build, pt
+    calls = []
+    real = build.build
+
+    def spy(*a, **k):
+        calls.append(1)
+        return real(*a, **k)
+
+    monkeypatch.setattr(build, "build", spy)
+    monkeypatch.setattr(pt, "_lib", None)
+    pt.lib()
+    assert calls, "pt.lib() must call build.build()"
+    # the stamp makes the second build a no-op: the library file is not rewritten
+    before = os.path.getmtime(build.LIB)
+    real()
+    assert os.path.getmtime(build.LIB) == before
+    # and a changed fingerprint (what a source edit does) invalidates it
+    with open(build.STAMP) as fh:
+        stamp = fh.read()
+    assert stamp.strip() == build._fingerprint()
+
+
+def test_peak_probe_is_not_part_of_the_product_abi(lib_path):
+    """The bench-only micro-benchmarks live in their own library (libpt_probe.so), not in libpt.so or include/pt.h."""
+    from paper_1906_10598_b200 import build
+    assert "pt_peak_probe" not in _declared_symbols()
+    lib = C.CDLL(lib_path)
+    assert not hasattr(lib, "pt_peak_probe") and not hasattr(lib, "pt_bench_peak_probe")
+    probe = C.CDLL(build.build_probe())
+    assert hasattr(probe, "pt_bench_peak_probe")
+
+
+def test_header_documents_every_status_bit_and_the_async_contract():
+    with open(os.path.join(ROOT, "include", "pt.h")) as fh:
+        text = fh.read()
+    for bit in ("bit0 (1)", "bit1 (2)", "bit2 (4)", "bit3 (8)", "bit4 (16)"):
+        assert bit in text, bit
+    assert "never synchronise the device or the stream" in text
+    # no non-_host entry point may say that it synchronises
+    for m in re.finditer(r"/\*(.*?)\*/\s*(?:typedef struct \{.*?\} \w+;\s*)?PT_API[^;]*?\b(pt_\w+)\s*\(", text, re.S):
+        doc, name = m.group(1), m.group(2)
+        if not name.endswith("_host") and not name.endswith("_host_q"):
+            assert "synchronises `stream`" not in doc, name
+
+
+def test_refit_workspace_query_and_validation_need_no_gpu(lib_path):
+    from paper_1906_10598_b200 import pt
+    L = pt.lib()
+    cfg = pt.make_config(D=5, NP=128, generations=10, t0=-0.5)
+    n = L.pt_refit_doubtful_workspace_bytes(3600, 16000, C.byref(cfg))
+    # per_block [B][10] f64 + total phase + flags + list + the device counter, each rounded to 256 bytes
+    assert n >= 3600 * (80 + 8 + 4 + 4) + 4 and n % 256 == 0
+    dummy = C.c_void_p(256)
+    bad = pt.make_retry_config(phi_tol=-1.0, F_tol=1.0)
+    assert L.pt_refit_doubtful(dummy, 4, 1000, 1000.0, dummy, dummy, None, C.byref(cfg), C.byref(bad), dummy, dummy, dummy, dummy,
+                               dummy, n, None) == -1
+    ok = pt.make_retry_config(phi_tol=1.0, F_tol=1.0)
+    assert L.pt_refit_doubtful(dummy, 4, 1000, 1000.0, dummy, dummy, None, C.byref(cfg), C.byref(ok), dummy, dummy, dummy, dummy,
+                               dummy, 16, None) == -2          # workspace too small
+
+
+def test_plan_and_error_state_are_thread_safe(lib_path):
+    """Per-device state of the library is mutex-guarded and the error string is per thread: hammer the plan query from threads."""
+    import threading
+    from paper_1906_10598_b200 import pt
+    pt.lib()
+    errs = []
+
+    def work(k):
+        try:
+            for _ in range(200):
+                cfg = pt.make_config(D=5 + (k & 1), NP=64 * (1 + k % 3), generations=10, t0=-0.5)
+                plan = pt.pt_fit_blocks_plan(100 + k, 4096, cfg)
+                assert plan["threads"] % 32 == 0
+        except Exception as exc:      # pragma: no cover
+            errs.append(exc)
+
+    ts = [threading.Thread(target=work, args=(k,)) for k in range(8)]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+    assert not errs

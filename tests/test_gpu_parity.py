@@ -463,13 +463,13 @@ def test_fit_config3_blocks(pt):
     o = _oracle_fit(wl, seed=4)
     dphi = _wrap(g["best"][:, 2] - o["best"][:, 2])
     assert np.max(np.abs(dphi)) < PHI0_TOL
-    # DESIGN.md R20: with T = 0.1 s the Cramer-Rao sigma of f is 4.4e-2 Hz and a change of f by 1e-3 Hz moves the RSS
-    # by 1e-7 relative -- one ulp of the fp32 objective (R18) -- so the fp32 and fp64 fits agree on f to a tenth of
-    # the statistical sigma, not to the 1e-3 Hz that north_star quotes for the 1-s blocks.
+    # north_star's |df| < 1e-3 Hz holds as it stands on blocks at the configured SNR (block 100; measured on 95 + 25 blocks in
+    # tests/test_gpu_oracle_subset.py).  Block 17950 sits at the bottom of the amplitude fade (a0 = 0.105, -10 dB per sample):
+    # there the chi^2 surface is flatter than the fp32 objective resolves and the bar is max(1e-3 Hz, 0.01 sigma_f) (R20).
     T = wl.T
     for k in range(wl.B):
         sig_f = _crlb(wl.truth[k], wl.N, wl.fs, wl.meta["sigma_per_block"][k] if "sigma_per_block" in wl.meta else wl.sigma, 6)[3]
-        f_tol = max(F_TOL, 0.1 * sig_f)
+        f_tol = F_TOL if wl.truth[k, 0] >= 0.3 else max(F_TOL, 0.01 * sig_f)
         assert abs(g["best"][k, 3] - o["best"][k, 3]) < f_tol, (k, f_tol)
         inc_g = 2 * np.pi * (g["best"][k, 3] * T + g["best"][k, 5] * T**3 / 24)
         inc_o = 2 * np.pi * (o["best"][k, 3] * T + o["best"][k, 5] * T**3 / 24)
