@@ -79,6 +79,14 @@ def make_workload(name: str, case: int):
         return W.config3(blocks=range(16200, 19800), case=case)
     if name == "config2_ncu":    # one wave of config-2 blocks, 100 generations: short enough for `ncu --set full`
         return W.config2(blocks=range(148), case=case, generations=100)
+    if name == "config3_ncu":    # one wave of config-3 blocks (D = 6) around the occultation, 100 generations
+        return W.config3(blocks=range(17926, 18074), case=case, generations=100)
+    if name == "config2_2w":     # two waves of config-2 blocks (the tensor-core kernel fits two blocks per CTA at a time)
+        return W.config2(blocks=range(296), case=case, generations=100)
+    if name == "config3_2w":
+        return W.config3(blocks=range(17852, 18148), case=case, generations=100)
+    if name == "config3":        # BASELINE config 3 at full size: 36000 blocks x 10000 samples, D = 6, 1500 generations
+        return W.config3(case=case)
     if name == "paper":          # the paper's own block shape and Table 4 settings
         return W.paper_blocks(B=148, case=case)
     if name == "tiny":           # for CPU-side plumbing tests
@@ -299,6 +307,8 @@ def main():
                     help="feed packed samples of this many bits (Table 3 formats, pt_fit_blocks_q / pt_track_host_q)")
     ap.add_argument("--fix-a1", action="store_true", help="fix the amplitude slope at zero (a1 box [0, 0], PAPER.md:139)")
     ap.add_argument("--objective", default="chi2", choices=["chi2", "cor"], help="Eq. 4 (default) or Eq. 5-6")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "tc", "classic"],
+                    help="force the tensor-core (pt_tc_kernel) or the FP32-pipe (pt_block_kernel) evaluation kernel (PT_KERNEL hook)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--sweep-n", default="1024,4096,16384,65536,262144")
@@ -307,6 +317,8 @@ def main():
     ap.add_argument("--sweep-generations", type=int, default=200)
     args = ap.parse_args()
 
+    if args.kernel != "auto":
+        os.environ["PT_KERNEL"] = args.kernel
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -428,8 +440,9 @@ def main():
                 # (a committed profile, not this run) ride along as traffic_ncu
                 "traffic": algorithmic_traffic(wl, args.quant),
                 "traffic_ncu": NCU_TRAFFIC.get(args.workload) if not (wl.de["objective"] or args.quant or args.strategy) else None,
-                "kernel": "pt_block_kernel<C=%d,D=%d,fit,%s>" % (plan["cands_per_thread"], wl.de["D"],
-                                                                "cor" if wl.de["objective"] else "chi2"),
+                "kernel": ("pt_tc_kernel<D=%d,fit,%s> (phase by tcgen05.mma kind::tf32)" % (wl.de["D"], "cor" if wl.de["objective"] else "chi2"))
+                if plan["threads"] == 640 else
+                "pt_block_kernel<C=%d,D=%d,fit,%s>" % (plan["cands_per_thread"], wl.de["D"], "cor" if wl.de["objective"] else "chi2"),
                 "kernel_ms": fit_ms, "peak_source": "derived: 148 SMs x 16 MUFU lanes x 1965 MHz (DESIGN.md); "
                 "MEASURED_PEAKS.json holds no ALU peak",
                 "frac_at_sampled_clock": achieved / (SM_COUNT * XU_LANES_PER_SM * sm_mhz * 1e6),

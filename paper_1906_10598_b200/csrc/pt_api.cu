@@ -10,6 +10,7 @@
 
 #include "../../include/pt.h"
 #include "pt_de_kernel.cuh"
+#include "pt_tc_kernel.cuh"
 #include "pt_internal.h"
 
 namespace pt {
@@ -37,6 +38,8 @@ struct Plan {
     int TS, S;              // streamed path: samples per tile, ring stages (0, 0 when resident)
     size_t ws_bytes;        // device workspace the launch needs (streamed path only)
     int K, NpadS;           // cluster path: CTAs per block, padded samples of the largest slice (K = 1: Npad)
+    int tc;                 // 1: the tensor-core kernel (pt_tc_kernel.cuh) fits these blocks
+    int tc_slots;           //    data blocks one of its CTAs fits at the same time (2 when shared memory allows)
 };
 
 // Per-device facts and per-device launch attributes, keyed by the CUDA device ordinal and guarded by one mutex: a process may
@@ -75,10 +78,30 @@ static void choose_warp_grid(int warps, int groups, int nch, int* Wg, int* Ws) {
     }
 }
 
+// Which evaluation kernel fits a block: pt_block_kernel (phase on the FP32 pipe) or pt_tc_kernel (phase on the tensor cores).
+// Automatic choice = whichever measured faster on the B200: the tensor-core kernel for D = 6 under chi^2 with
+// a population that fills at least three quarters of its 128 candidate lanes.  PT_KERNEL=tc / PT_KERNEL=classic in the
+// environment forces one of them where it applies (tests, A/B measurements); unset = automatic.
+static int kernel_override() {
+    const char* e = getenv("PT_KERNEL");
+    if (!e || !*e) return 0;
+    if (!strcmp(e, "tc")) return 1;
+    if (!strcmp(e, "classic")) return 2;
+    return 0;
+}
+static bool want_tc(int NP, int D, int objective) {
+    if (NP > kTcMaxNP) return false;
+    const int o = kernel_override();
+    if (o == 1) return true;
+    if (o == 2) return false;
+    return D == 6 && objective == kObjChi2 && NP >= 96;
+}
+
 // sms / smem_optin are passed in so that the plan can also be computed without a device (defaults of B200).
 // force_K > 0 overrides the cluster-size choice (tests, tuning); 0 = automatic
-static int make_plan(long long B, int N, int NP, int D, int sms, int smem_optin, int force_K, Plan* pl) {
+static int make_plan(long long B, int N, int NP, int D, int sms, int smem_optin, int force_K, Plan* pl, int objective = 0) {
     pl->sms = sms;
+    pl->tc = 0; pl->tc_slots = 1;
     pl->C = (NP % 8 == 0) ? 8 : 4;
     pl->NPpad = (NP + pl->C - 1) / pl->C * pl->C;
     pl->Npad = (N + kChunk - 1) / kChunk * kChunk;
@@ -106,6 +129,17 @@ static int make_plan(long long B, int N, int NP, int D, int sms, int smem_optin,
                 pl->grid = (int)((long long)B * K < want ? (long long)B * K : want);
                 return 0;
             }
+        }
+    }
+    if (want_tc(NP, D, objective)) {
+        // one CTA of 640 threads per SM; shared memory holds the samples only, so the block must be resident
+        for (int slots = 2; slots >= 1; --slots) {
+            const TcSmemLayout L(N, NP, D, slots);
+            if (L.total > smem_optin) continue;
+            pl->tc = 1; pl->tc_slots = slots; pl->C = 1; pl->NPpad = kTcMaxNP; pl->threads = kTcThreads; pl->Wg = 4; pl->Ws = 4;
+            pl->ctas_per_sm = 1; pl->smem = L.total; pl->resident = 1; pl->TS = 0; pl->S = 0; pl->ws_bytes = 0;
+            pl->grid = (int)(B < sms ? B : sms);
+            return 0;
         }
     }
     for (int cps = 4; cps >= 1; cps >>= 1) {
@@ -151,7 +185,7 @@ static int force_cluster() {
 }
 
 // plan with the current device's limits, or B200's when no device is present (the query entry points)
-static int plan_for(long long B, int N, int NP, int D, Plan* pl, bool need_device, int force_K = 0) {
+static int plan_for(long long B, int N, int NP, int D, Plan* pl, bool need_device, int force_K = 0, int objective = 0) {
     int sms = 148, smem_optin = 232448;
     int dev_count = 0;
     if (cudaGetDeviceCount(&dev_count) == cudaSuccess && dev_count > 0) {
@@ -160,7 +194,7 @@ static int plan_for(long long B, int N, int NP, int D, Plan* pl, bool need_devic
         (void)cudaGetLastError();
         if (need_device) { set_error("no CUDA device"); return PT_ERR_CUDA; }
     }
-    if (make_plan(B, N, NP, D, sms, smem_optin, force_K > 0 ? force_K : force_cluster(), pl)) {
+    if (make_plan(B, N, NP, D, sms, smem_optin, force_K > 0 ? force_K : force_cluster(), pl, objective)) {
         set_error("N = %d with NP = %d: population tables alone exceed shared memory", N, NP);
         return PT_ERR_UNSUPPORTED;
     }
@@ -244,8 +278,34 @@ static int dispatch2(const BlockParams& p, const Plan& pl, int D, int objective,
     return objective == kObjCor ? dispatch3<MODE, STREAM, kObjCor>(p, pl, D, st) : dispatch3<MODE, STREAM, kObjChi2>(p, pl, D, st);
 }
 
+template <int D, int MODE, int OBJ>
+static int launch_tc_kernel(const BlockParams& p, const Plan& pl, cudaStream_t st) {
+    static int configured_smem[kMaxDevices];
+    int dev = 0;
+    if (check_cuda(cudaGetDevice(&dev), "cudaGetDevice")) return PT_ERR_CUDA;
+    if (dev < 0 || dev >= kMaxDevices) { set_error("device ordinal %d beyond the compiled limit %d", dev, kMaxDevices); return PT_ERR_CUDA; }
+    {
+        std::lock_guard<std::mutex> lock(g_dev_mutex);
+        if (pl.smem > configured_smem[dev]) {
+            if (check_cuda(cudaFuncSetAttribute(pt_tc_kernel<D, MODE, OBJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem), "cudaFuncSetAttribute"))
+                return PT_ERR_CUDA;
+            configured_smem[dev] = pl.smem;
+        }
+    }
+    pt_tc_kernel<D, MODE, OBJ><<<pl.grid, pl.threads, pl.smem, st>>>(p);
+    if (check_cuda(cudaGetLastError(), "pt_tc_kernel launch")) return PT_ERR_CUDA;
+    return PT_OK;
+}
+
+template <int MODE>
+static int dispatch_tc(const BlockParams& p, const Plan& pl, int D, int objective, cudaStream_t st) {
+    if (objective == kObjCor) return D == 5 ? launch_tc_kernel<5, MODE, kObjCor>(p, pl, st) : launch_tc_kernel<6, MODE, kObjCor>(p, pl, st);
+    return D == 5 ? launch_tc_kernel<5, MODE, kObjChi2>(p, pl, st) : launch_tc_kernel<6, MODE, kObjChi2>(p, pl, st);
+}
+
 template <int MODE>
 static int dispatch(const BlockParams& p, const Plan& pl, int D, int objective, cudaStream_t st) {
+    if (pl.tc) return dispatch_tc<MODE>(p, pl, D, objective, st);
     return pl.S > 0 ? dispatch2<MODE, true>(p, pl, D, objective, st) : dispatch2<MODE, false>(p, pl, D, objective, st);
 }
 
@@ -276,7 +336,7 @@ static long long plan_tail(long long B, int N, int NP, int D, const Plan& pl, Pl
 // streamed path: hand the workspace rows to the kernel
 static int attach_workspace(BlockParams* p, const Plan& pl, void* workspace, size_t workspace_bytes) {
     p->TS = pl.TS; p->S = pl.S;
-    p->K = pl.K; p->NpadS = pl.NpadS;
+    p->K = pl.K; p->NpadS = pl.NpadS; p->tc_slots = pl.tc_slots;
     if (pl.S == 0) return PT_OK;
     if (!workspace || workspace_bytes < pl.ws_bytes) {
         set_error("streamed path (N = %d does not fit in shared memory) needs %zu bytes of workspace, got %zu", p->N, pl.ws_bytes,
@@ -391,7 +451,7 @@ int32_t pt_objective(const float* x, int64_t B, int32_t N, double fs, double t0,
     if (!std::isfinite(t0)) { set_error("t0 must be finite"); return PT_ERR_INVALID_ARG; }
     if (objective != PT_OBJECTIVE_CHI2 && objective != PT_OBJECTIVE_COR) { set_error("objective must be 0 (chi^2) or 1 (correlation), got %d", objective); return PT_ERR_INVALID_ARG; }
     Plan pl;
-    rc = plan_for(B, N, NP, D, &pl, true);
+    rc = plan_for(B, N, NP, D, &pl, true, 0, objective);
     if (rc) return rc;
     BlockParams p;
     memset(&p, 0, sizeof(p));
@@ -411,7 +471,7 @@ int32_t pt_fitness(const float* x, int64_t B, int32_t N, double fs, double t0, c
 
 size_t pt_fit_blocks_workspace_bytes(int64_t B, int32_t N, const pt_de_config* cfg) {
     Plan pl;
-    if (!cfg || check_common(B, N, 1.0, cfg->NP, cfg->D) || plan_for(B, N, cfg->NP, cfg->D, &pl, false)) return 0;
+    if (!cfg || check_common(B, N, 1.0, cfg->NP, cfg->D) || plan_for(B, N, cfg->NP, cfg->D, &pl, false, 0, cfg->objective)) return 0;
     return pl.ws_bytes;
 }
 
@@ -420,7 +480,7 @@ int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg, int32_
     int rc = check_common(B, N, 1.0, cfg->NP, cfg->D);
     if (rc) return rc;
     Plan pl;
-    rc = plan_for(B, N, cfg->NP, cfg->D, &pl, false);
+    rc = plan_for(B, N, cfg->NP, cfg->D, &pl, false, 0, cfg->objective);
     if (rc) return rc;
     out[0] = pl.grid; out[1] = pl.threads; out[2] = pl.smem; out[3] = pl.resident; out[4] = pl.C; out[5] = pl.ctas_per_sm;
     out[6] = pl.K; out[7] = 0;
@@ -454,7 +514,7 @@ static int32_t fit_blocks_impl(const float* x, const unsigned char* xq, const pt
         if (rc) return rc;
     }
     Plan pl;
-    rc = plan_for(B, N, cfg->NP, cfg->D, &pl, true, count ? 1 : 0);
+    rc = plan_for(B, N, cfg->NP, cfg->D, &pl, true, count ? 1 : 0, cfg->objective);
     if (rc) return rc;
     p.x = x; p.xq = xq; p.row_bytes = row_bytes;
     p.lo = lo; p.hi = hi; p.block_index = block_index; p.sel = sel; p.count = count;
@@ -546,7 +606,7 @@ static void refit_layout(int64_t B, size_t fit_ws, size_t* o_pb, size_t* o_tp, s
 // workspace of the re-fit launches: the plan of B single-CTA blocks (see fit_blocks_impl, count != null)
 static size_t refit_fit_workspace_bytes(int64_t B, int32_t N, const pt_de_config* cfg) {
     Plan pl;
-    if (!cfg || check_common(B, N, 1.0, cfg->NP, cfg->D) || plan_for(B, N, cfg->NP, cfg->D, &pl, false, 1)) return 0;
+    if (!cfg || check_common(B, N, 1.0, cfg->NP, cfg->D) || plan_for(B, N, cfg->NP, cfg->D, &pl, false, 1, cfg->objective)) return 0;
     return pl.ws_bytes;
 }
 

@@ -74,6 +74,7 @@ struct BlockParams {
     // candidate over that slice, and the K partial sums of every candidate are exchanged through distributed shared
     // memory; the DE step itself is replicated (counter-based RNG, fp64: bit-identical in every CTA).
     int K;                        // CTAs per cluster = per block; 1: no cluster
+    int tc_slots;                 // pt_tc_kernel: data blocks a CTA fits at the same time (1 or 2)
     int NpadS;                    // padded samples of the largest slice (= Npad when K == 1)
 };
 
