@@ -537,7 +537,7 @@ static int32_t fit_blocks_impl(const float* x, const unsigned char* xq, const pt
     if (rc) return rc;
     BlockParams q = p;
     q.blk0 = B - rem; q.B = B;
-    q.Wg = tl.Wg; q.Ws = tl.Ws;
+    q.Wg = tl.Wg; q.Ws = tl.Ws; q.Npad = tl.Npad; q.NPpad = tl.NPpad;   // the tail plan is always pt_block_kernel's
     rc = attach_workspace(&q, tl, nullptr, 0);
     if (rc) return rc;
     return dispatch<kModeFit>(q, tl, cfg->D, cfg->objective, (cudaStream_t)stream);

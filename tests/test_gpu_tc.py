@@ -214,3 +214,29 @@ def test_classic_kernel_still_covers_d6(pt):
             assert abs(float(r["best_rss"][k]) - v) / v < FIT_REL_TOL
     assert np.abs(_wrap(a["best"][:, 2] - b["best"][:, 2])).max() < PHI0_TOL
     assert np.abs(a["best"][:, 3] - b["best"][:, 3]).max() < F_TOL
+
+
+def test_tc_main_launch_with_classic_cluster_tail(pt):
+    """B = 2 waves + a short tail: full waves on the tensor-core kernel (two blocks per CTA), the tail on clusters of the FP32-pipe
+    kernel (two launches).  Every block must equal its single-block fit up to the summation order of its kernel."""
+    wl = W.single_tone_blocks(range(310), 512, 512.0, config=4, f_range=(20, 60))
+    wl.de = dict(NP=16, D=5, generations=6, F=0.5, CR=0.9)
+    cfg = pt.make_config(D=5, NP=16, generations=6, seed=9, t0=wl.t0)
+    old = os.environ.get("PT_KERNEL")
+    os.environ["PT_KERNEL"] = "tc"
+    try:
+        plan = pt.pt_fit_blocks_plan(wl.B, wl.N, cfg)
+        assert plan["threads"] == 640 and plan["tail_cluster"] >= 2, plan
+        r = pt.pt_fit_blocks(_cuda(wl.x), wl.fs, _cuda(wl.lo), _cuda(wl.hi), cfg, want_pop=True)
+        torch.cuda.synchronize()
+    finally:
+        if old is None:
+            os.environ.pop("PT_KERNEL", None)
+        else:
+            os.environ["PT_KERNEL"] = old
+    g = {k: v.cpu().numpy() for k, v in r.items()}
+    assert np.all(np.isfinite(g["best_rss"])) and np.all(g["best"] >= wl.lo) and np.all(g["best"] <= wl.hi)
+    o = oracle.fit_blocks(wl.x[[0, 200, 305]], wl.fs, wl.lo[[0, 200, 305]], wl.hi[[0, 200, 305]], NP=16, generations=6, seed=9,
+                          block_index=np.array([0, 200, 305], dtype=np.uint32), want_pop=True)
+    same = np.all(g["final_pop"][[0, 200, 305]] == o["final_pop"].astype(np.float32), axis=-1)
+    assert same.mean() > 0.9
