@@ -81,6 +81,14 @@ def make_workload(name: str, case: int):
         return W.config2(blocks=range(148), case=case, generations=100)
     if name == "config3_ncu":    # one wave of config-3 blocks (D = 6) around the occultation, 100 generations
         return W.config3(blocks=range(17926, 18074), case=case, generations=100)
+    if name == "paper_ncu":      # paper-shaped blocks (streamed, D = 6, NP = 400), 10 generations: short enough for `ncu --set full`
+        wl = W.paper_blocks(B=148, case=case)
+        wl.de["generations"] = 10
+        return wl
+    if name == "config1_ncu":    # config 1 (60 blocks: clusters of 2 CTAs per block), 100 generations
+        return W.config1(case=case, generations=100)
+    if name == "sweep1k_ncu":    # config-4 sweep point N = 1024, NP = 128 (4 CTAs per SM)
+        return W.config4(1024, 128, B=1024, generations=200)
     if name == "config2_2w":     # two waves of config-2 blocks (the tensor-core kernel fits two blocks per CTA at a time)
         return W.config2(blocks=range(296), case=case, generations=100)
     if name == "config3_2w":
@@ -283,6 +291,89 @@ def run_sweep(args, dev):
     print(json.dumps(line), flush=True)
 
 
+def run_strong(args, rank: int, local_rank: int, world: int, dev):
+    """--scaling strong: one track (config2 / config3 / config3s) split over the ranks.  Each rank synthesises and fits only its
+    contiguous range of blocks (the Philox counter carries the block's index in the full track, so the split draws the random
+    numbers of the unsplit fit); the one exchange of the path is the all-gather of best[B][D] before the Doppler products."""
+    import torch
+    import torch.distributed as dist
+    from paper_1906_10598_b200 import pt, shard, workloads as W
+    if not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29541")
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=dev)
+    full = {"config2": (W.config2, range(3600)), "config3": (W.config3, range(36000)), "config3s": (W.config3, range(16200, 19800)),
+            "tiny": (lambda **k: W.config2(generations=3, **k), range(8))}
+    if args.workload not in full:
+        raise SystemExit("--scaling strong takes --workload config2 | config3 | config3s")
+    make, blocks = full[args.workload]
+    blocks = list(blocks)
+    B = len(blocks)
+    mine = shard.block_range(B, rank, world)
+    wl = apply_variant(make(blocks=[blocks[k] for k in mine]), args.strategy, args.objective, args.fix_a1)
+    cfg = pt.make_config(D=wl.de["D"], NP=wl.de["NP"], generations=wl.de["generations"], F=wl.de["F"], CR=wl.de["CR"], seed=1,
+                         t0=wl.t0, strategy=wl.de["strategy"], objective=wl.de["objective"])
+    m_int = [max(1, int(round(tc / wl.T))) for tc in (1.0, 10.0, 60.0)]
+    x_h, lo_h, hi_h = (torch.from_numpy(a).pin_memory() for a in (wl.x, wl.lo, wl.hi))
+    x, lo, hi = x_h.to(dev), lo_h.to(dev), hi_h.to(dev)
+    units = float(B) * wl.de["NP"] * (wl.de["generations"] + 1) * wl.N
+
+    def step(xd, lod, hid):
+        r = shard.fit_track_sharded(xd, wl.fs, lod, hid, cfg, B)          # block_index = position in the full track
+        return r, pt.pt_doppler_products(r["best"], wl.T, 0.0, m_int)
+
+    def barrier():
+        dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step(x, lo, hi)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        r, prod = step(x, lo, hi)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    tt = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    ms_per_step = float(tt.item()) / args.steps
+    # end to end: this rank's samples from pinned host memory, sharded fit, products, results back on the host
+    barrier()
+    t0 = time.perf_counter()
+    n_e2e = max(1, min(args.steps, 2))
+    for _ in range(n_e2e):
+        r, prod = step(x_h.to(dev, non_blocking=True), lo_h.to(dev, non_blocking=True), hi_h.to(dev, non_blocking=True))
+        out = [r["best"].cpu(), r["best_rss"].cpu(), r["status"].cpu(), prod[0].cpu(), prod[1].cpu()] + [v.cpu() for v in prod[2]]
+    barrier()
+    tt = torch.tensor([(time.perf_counter() - t0) / n_e2e], dtype=torch.float64, device=dev)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    e2e_s = float(tt.item())
+    if rank == 0:
+        value = units / (ms_per_step * 1e-3)
+        cfgd = workload_config(args.workload, wl)
+        cfgd["blocks"] = B
+        cfgd["parallelism"] = ("one track split into contiguous block ranges over %d rank(s); one all-gather of best[B][D] (%.2f MB, NCCL) "
+                               "before the Doppler products" % (world, B * wl.de["D"] * 8 / 1e6))
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+                "data": "synthetic", "config": cfgd, "real_time_factor": B * wl.T / (ms_per_step * 1e-3),
+                "roofline": {"bound": "alu", "achieved": value / 1e12, "peak": world * XU_PEAK / 1e12,
+                             "unit": "T sample-evals/s (1 MUFU cosine each)", "frac": value / (world * XU_PEAK),
+                             "traffic": algorithmic_traffic(wl) * B / max(1, wl.B)},
+                "clocks": clocks,
+                "e2e": {"value": units / e2e_s, "unit": UNIT, "ms_per_step": 1e3 * e2e_s,
+                        "h2d_bytes_per_step": int(sum(t.numel() * t.element_size() for t in (x_h, lo_h, hi_h))),
+                        "d2h_bytes_per_step": int(sum(t.numel() * t.element_size() for t in out))},
+                "gpu_launches": args.steps * (2 + 2 + len([m for m in m_int if B // m > 0]))}
+        print(json.dumps(line), flush=True)
+    dist.destroy_process_group()
+
+
 def workload_config(name: str, wl, full=True) -> dict:
     return {"workload": "BASELINE.json config 2 (one-hour track)" if name == "config2" else name,
             "strategy": wl.de.get("strategy", 1), "a1": "fixed at 0" if wl.meta.get("fix_a1") else "free", "objective": "cor (Eq. 5-6)" if wl.de.get("objective", 0) else "chi2 (Eq. 4)",
@@ -309,6 +400,9 @@ def main():
     ap.add_argument("--objective", default="chi2", choices=["chi2", "cor"], help="Eq. 4 (default) or Eq. 5-6")
     ap.add_argument("--kernel", default="auto", choices=["auto", "tc", "classic"],
                     help="force the tensor-core (pt_tc_kernel) or the FP32-pipe (pt_block_kernel) evaluation kernel (PT_KERNEL hook)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="weak: every rank fits its own track (default); strong: ONE track split into contiguous block ranges over "
+                         "the ranks (shard.fit_track_sharded), all-gather of the fitted parameters before the Doppler products")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--sweep-n", default="1024,4096,16384,65536,262144")
@@ -344,6 +438,9 @@ def main():
         if world > 1:
             raise SystemExit("--workload sweep is a 1-GPU report")
         run_sweep(args, dev)
+        return
+    if args.scaling == "strong":
+        run_strong(args, rank, local_rank, world, dev)
         return
     wl = apply_variant(make_workload(args.workload, case=rank), args.strategy, args.objective, args.fix_a1)   # every rank fits its own track
     cfg = pt.make_config(D=wl.de["D"], NP=wl.de["NP"], generations=wl.de["generations"], F=wl.de["F"], CR=wl.de["CR"],

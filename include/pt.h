@@ -14,8 +14,9 @@
  *     pt_last_error_string() describes the last failure of the calling thread.
  *   - Unless a parameter is marked [host], every array pointer is a DEVICE pointer owned by the caller
  *     (the Python binding allocates them with torch).  Layouts are dense row-major.  Inputs are never
- *     modified.  The library keeps no device memory between calls; scratch is passed in by the caller and
- *     sized by the *_workspace_bytes query.
+ *     modified.  The device entry points keep no device memory between calls; scratch is passed in by the caller
+ *     and sized by the *_workspace_bytes query.  (The *_host entry points keep a stream-ordered memory pool and a
+ *     stream per device between calls, so that a repeated call pays no cudaMalloc; pt_host_cache_release() frees them.)
  *   - Device entry points are asynchronous on the given stream and never synchronise the device or the stream.
  *     The *_host entry points are synchronous and own their temporary device memory.
  *   - One process may drive several devices from several host threads: per-device state inside the library is keyed by
@@ -281,6 +282,10 @@ PT_API int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, co
                       const pt_de_config* cfg, double los_scale, const int32_t* blocks_per_interval,
                       int32_t n_intervals, double* best, float* best_rss, uint32_t* status, double* per_block,
                       double* total_phase, double* const* interval_out);
+
+/* pt_host_cache_release -- destroys the per-device memory pools and streams the *_host entry points keep between calls
+ * (synchronises those streams).  The next *_host call creates them again.  Returns PT_OK or PT_ERR_CUDA. */
+PT_API int32_t pt_host_cache_release(void);
 
 /* pt_track_host_q -- pt_track_host on quantised HOST samples xq[B][row_bytes] (see pt_quant): the host-to-device copy
  * moves the packed bytes (bits/32 of the fp32 volume). */

@@ -49,6 +49,35 @@ static std::mutex g_dev_mutex;
 struct DeviceFacts { int known, sms, smem_optin; };
 static DeviceFacts g_dev[kMaxDevices];
 
+// *_host entry points: a stream-ordered memory pool and a stream per device, kept between calls so that a repeated call pays
+// neither cudaMalloc / cudaFree (0.5 ms each, with occasional outliers of 10-100 ms) nor stream creation.
+struct HostCache { int ready; cudaMemPool_t pool; cudaStream_t stream; };
+static HostCache g_host_cache[kMaxDevices];
+
+static int host_cache_get(cudaMemPool_t* pool, cudaStream_t* stream) {
+    int dev = 0;
+    if (check_cuda(cudaGetDevice(&dev), "cudaGetDevice")) return 1;
+    if (dev < 0 || dev >= kMaxDevices) { set_error("device ordinal %d beyond the compiled limit %d", dev, kMaxDevices); return 1; }
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    HostCache& c = g_host_cache[dev];
+    if (!c.ready) {
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof(props));
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        if (check_cuda(cudaMemPoolCreate(&c.pool, &props), "cudaMemPoolCreate")) return 1;
+        unsigned long long keep = ~0ull;        // freed blocks stay in the pool until pt_host_cache_release()
+        if (check_cuda(cudaMemPoolSetAttribute(c.pool, cudaMemPoolAttrReleaseThreshold, &keep), "cudaMemPoolSetAttribute")) return 1;
+        if (check_cuda(cudaStreamCreateWithFlags(&c.stream, cudaStreamNonBlocking), "cudaStreamCreate")) return 1;
+        c.ready = 1;
+    }
+    *pool = c.pool;
+    *stream = c.stream;
+    return 0;
+}
+
 static int device_info(int* sms, int* smem_optin, int* dev_out = nullptr) {
     int dev = 0;
     if (check_cuda(cudaGetDevice(&dev), "cudaGetDevice")) return 1;
@@ -759,10 +788,11 @@ static int32_t track_host_impl(const float* x, const void* xq, const pt_quant* q
         cnt[k] = B / blocks_per_interval[k];
         o_iv[k] = take((size_t)(cnt[k] > 0 ? cnt[k] : 1) * 16);
     }
-    unsigned char* arena = nullptr;
-    if (check_cuda(cudaMalloc(&arena, off), "cudaMalloc")) return PT_ERR_CUDA;
+    cudaMemPool_t pool;
     cudaStream_t st = nullptr;
-    if (check_cuda(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking), "cudaStreamCreate")) { cudaFree(arena); return PT_ERR_CUDA; }
+    if (host_cache_get(&pool, &st)) return PT_ERR_CUDA;
+    unsigned char* arena = nullptr;
+    if (check_cuda(cudaMallocFromPoolAsync(reinterpret_cast<void**>(&arena), off, pool, st), "cudaMallocFromPoolAsync")) return PT_ERR_CUDA;
     int ret = PT_OK;
     std::vector<double*> d_iv(n_intervals > 0 ? n_intervals : 1, nullptr);
     for (int k = 0; k < n_intervals; ++k) d_iv[k] = reinterpret_cast<double*>(arena + o_iv[k]);
@@ -810,9 +840,26 @@ static int32_t track_host_impl(const float* x, const void* xq, const pt_quant* q
         if (check_cuda(cudaStreamSynchronize(st), "pt_track_host")) { ret = PT_ERR_CUDA; break; }
     } while (0);
     if (ret != PT_OK) cudaStreamSynchronize(st);
-    cudaStreamDestroy(st);
-    cudaFree(arena);
+    cudaFreeAsync(arena, st);            // back to the pool (kept for the next call); ordered after everything above
     return ret;
+}
+
+int32_t pt_host_cache_release(void) {
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    int rc = PT_OK;
+    int cur = 0;
+    if (cudaGetDevice(&cur) != cudaSuccess) { (void)cudaGetLastError(); return PT_OK; }      // no device: nothing was ever cached
+    for (int dev = 0; dev < kMaxDevices; ++dev) {
+        HostCache& c = g_host_cache[dev];
+        if (!c.ready) continue;
+        cudaSetDevice(dev);
+        if (cudaStreamSynchronize(c.stream) != cudaSuccess) rc = PT_ERR_CUDA;
+        cudaStreamDestroy(c.stream);
+        cudaMemPoolDestroy(c.pool);
+        c.ready = 0;
+    }
+    cudaSetDevice(cur);
+    return rc;
 }
 
 int32_t pt_track_host(const float* x, int64_t B, int32_t N, double fs, const double* lo, const double* hi,

@@ -201,7 +201,7 @@ __device__ __forceinline__ void reduce_and_store(float (&acc)[C], const int lane
 
 // Not inlined on purpose: the loop's register allocation (which decides the operand-bank conflicts of the FFMA2 stream, the
 // binding resource of this loop) then does not depend on the code around it in the kernel.  Measured on config 2: 2101 ms
-// inlined vs 2071 ms as a call, with identical instruction mixes (profiles/r1d_codegen_ab.md).
+// inlined vs 2071 ms as a call, with identical instruction mixes.
 template <int C, int D, int OBJ>
 __device__ __noinline__ void eval_population(const BlockParams& p, const Slice& sl, const float* __restrict__ xs,
                                                 const float* __restrict__ wref, const float* __restrict__ cand,

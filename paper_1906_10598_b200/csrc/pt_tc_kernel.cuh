@@ -50,9 +50,9 @@ struct TcSmemLayout {
         s_popA = q; q += NP * D * 8;
         s_popT = q; q += NP * D * 8;
         s_box = q; q += 3 * 8 * 8;
-        s_fit = q; q += kTcMaxNP * 4;
+        s_fit = q; q += kTcMaxNP * 8;          // objective values of the members, fp64 (see tc_consumer_pass)
         s_amp = q; q += kTcMaxNP * 2 * 4;      // (-a0, -a1) of every member: what the consumers need of a candidate
-        s_part = q; q += 4 * kTcMaxNP * 4;     // [column group][candidate] partial sums
+        s_part = q; q += 4 * kTcMaxNP * 8;     // [column group][candidate] partial sums, fp64
         q = align_up(q, 16);
         s_xs = q; q += Npad * 4;
         slot_stride = align_up(q, 128);
@@ -105,10 +105,12 @@ struct TcConsumer {          // per-warp pipeline state of a consumer
 
 // Chunk K of a tile for a warp that owns 64 columns (four x16 loads through two 16-register buffers).  On entry chunk K is in
 // flight into `cur`; the next chunk (or chunk 0 of the next tile) is started into `nxt` before chunk K is evaluated.
-template <int AMP, int K>
+// INTERIOR: all 64 columns of the warp are samples of the block (every tile but the first and last of a block): no bounds
+// checks, and the amplitude runs on from chunk to chunk.
+template <int AMP, int K, bool INTERIOR>
 __device__ __forceinline__ void tc_tile_chunk(uint32_t (&cur)[16], uint32_t (&nxt)[16], TcConsumer& st, const float* __restrict__ xw,
-                                              const int n_first, const int N, const float g0w, const float g1, const f32x2 step, f32x2& acc,
-                                              const bool has_next) {
+                                              const int n_first, const int N, const float g0w, const float g1, f32x2& A2, const f32x2 step,
+                                              f32x2& acc, const bool has_next) {
     constexpr int nchunk = 4;
     tc::wait_ld();
     if (K == nchunk - 1) {
@@ -126,23 +128,32 @@ __device__ __forceinline__ void tc_tile_chunk(uint32_t (&cur)[16], uint32_t (&nx
     } else {
         tc::tmem_ld16(st.tbase + (st.it % tc::kTmemBufs) * tc::kTile + (K + 1) * 16, nxt);
     }
-    // sample index of the chunk's first column (a multiple of 16; negative or >= N: the chunk is padding and is skipped)
-    const int n0 = n_first + K * 16;
-    if (n0 >= 0 && n0 < N) {
-        // negated amplitude of the chunk's first two columns, then a running sum in steps of two columns
-        f32x2 A2 = (AMP == kTcAmpLinear) ? pack2(fmaf(g1, (float)(K * 16), g0w), fmaf(g1, (float)(K * 16 + 1), g0w)) : bc2(g0w);
-        if (n0 + 16 <= N) tc_consume16<AMP, false>(cur, xw + K * 16, A2, step, acc, 16);
-        else tc_consume16<AMP, true>(cur, xw + K * 16, A2, step, acc, N - n0);
+    if (INTERIOR) {
+        tc_consume16<AMP, false>(cur, xw + K * 16, A2, step, acc, 16);
+    } else {
+        // sample index of the chunk's first column (a multiple of 16; negative or >= N: the chunk is padding and is skipped)
+        const int n0 = n_first + K * 16;
+        if (n0 >= 0 && n0 < N) {
+            f32x2 Ac = (AMP == kTcAmpLinear) ? pack2(fmaf(g1, (float)(K * 16), g0w), fmaf(g1, (float)(K * 16 + 1), g0w)) : bc2(g0w);
+            if (n0 + 16 <= N) tc_consume16<AMP, false>(cur, xw + K * 16, Ac, step, acc, 16);
+            else tc_consume16<AMP, true>(cur, xw + K * 16, Ac, step, acc, N - n0);
+        }
     }
-    if constexpr (K + 1 < nchunk) tc_tile_chunk<AMP, K + 1>(nxt, cur, st, xw, n_first, N, g0w, g1, step, acc, has_next);
+    if constexpr (K + 1 < nchunk) tc_tile_chunk<AMP, K + 1, INTERIOR>(nxt, cur, st, xw, n_first, N, g0w, g1, A2, step, acc, has_next);
 }
 
 // One evaluation pass of a consumer warp over the block: sum over its 64 columns of every tile for its lane's candidate.
+// Summation: fp32 FMA accumulation over the thread's 64 columns of a tile (two packed accumulators of 32 terms), then an
+// error-free two-sum of the tile's value into a (hi, lo) pair -- 7 packed operations per tile and thread -- and fp64 from there
+// on (partials, the members' objective values, the selection).  A plain fp32 accumulator over a thread's N/4 terms would carry
+// ~1e-4 of absolute rounding at N = 10 000, two orders above what a 1e-3 Hz step of f moves the chi^2 of a faded block by
+// (R20).
 template <int AMP>
-__device__ __forceinline__ float tc_consumer_pass(TcConsumer& st, const float* __restrict__ xs, const int N, const int nT, const int c0,
-                                                  const int off, const float na0, const float na1, const float dtf, const float Ldtf,
-                                                  const float tw0) {
-    f32x2 acc = pack2(0.0f, 0.0f);
+__device__ __forceinline__ double tc_consumer_pass(TcConsumer& st, const float* __restrict__ xs, const int N, const int nT, const int c0,
+                                                   const int off, const float na0, const float na1, const float dtf, const float Ldtf,
+                                                   const float tw0) {
+    f32x2 hi = pack2(0.0f, 0.0f), lo = pack2(0.0f, 0.0f);
+    const f32x2 neg1 = bc2(-1.0f);
     uint32_t ua[16], ub[16];
     const float g1 = na1 * dtf;
     const f32x2 step = bc2(2.0f * g1);
@@ -156,33 +167,45 @@ __device__ __forceinline__ float tc_consumer_pass(TcConsumer& st, const float* _
         const float g0w = (AMP == kTcAmpLinear) ? fmaf(na1, fmaf(tauf, Ldtf, tw0), na0) : na0;
         tauf += 1.0f;
         const int col = tau * tc::kTile + c0;          // position of the warp's first column in the padded sample array
-        tc_tile_chunk<AMP, 0>(ua, ub, st, xs + col, col - off, N, g0w, g1, step, acc, tau + 1 < nT);
+        const int n_first = col - off;                 // its sample index
+        f32x2 A2 = (AMP == kTcAmpLinear) ? pack2(g0w, g0w + g1) : bc2(g0w);
+        f32x2 acc = pack2(0.0f, 0.0f);
+        if (n_first >= 0 && n_first + 64 <= N) tc_tile_chunk<AMP, 0, true>(ua, ub, st, xs + col, n_first, N, g0w, g1, A2, step, acc, tau + 1 < nT);
+        else tc_tile_chunk<AMP, 0, false>(ua, ub, st, xs + col, n_first, N, g0w, g1, A2, step, acc, tau + 1 < nT);
+        // (hi, lo) += acc without losing the rounding error of the addition (Knuth's two-sum, packed)
+        const f32x2 sum = add2(hi, acc);
+        const f32x2 bp = fma2(hi, neg1, sum);                              // sum - hi
+        const f32x2 e1 = fma2(fma2(bp, neg1, sum), neg1, hi);              // hi - (sum - bp)
+        const f32x2 e2 = fma2(bp, neg1, acc);                              // acc - bp
+        lo = add2(lo, add2(e1, e2));
+        hi = sum;
     }
-    float a0, a1;
-    unpack2(acc, a0, a1);
-    return a0 + a1;
+    float h0, h1, l0, l1;
+    unpack2(hi, h0, h1);
+    unpack2(lo, l0, l1);
+    return ((double)h0 + (double)h1) + ((double)l0 + (double)l1);
 }
 
 // argmin of fit[0..NP) with the lowest index on ties, and the maximum (a NaN is read as +inf); every lane gets them
-__device__ __forceinline__ void tc_warp_argmin(const float* fit, const int NP, const int lane, float& bv, int& bi, float& mx) {
-    bv = INFINITY; mx = -INFINITY; bi = 0x7fffffff;
+__device__ __forceinline__ void tc_warp_argmin(const double* fit, const int NP, const int lane, double& bv, int& bi, double& mx) {
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    bv = inf; mx = -inf; bi = 0x7fffffff;
     for (int i = lane; i < NP; i += 32) {
-        float v = fit[i];
-        if (!(v == v)) v = INFINITY;
+        double v = fit[i];
+        if (!(v == v)) v = inf;
         if (v < bv || (v == bv && i < bi)) { bv = v; bi = i; }
-        mx = fmaxf(mx, v);
+        mx = fmax(mx, v);
     }
 #pragma unroll
     for (int off = 16; off >= 1; off >>= 1) {
-        const float ov = __shfl_xor_sync(0xffffffffu, bv, off);
+        const double ov = __shfl_xor_sync(0xffffffffu, bv, off);
         const int oi = __shfl_xor_sync(0xffffffffu, bi, off);
-        const float om = __shfl_xor_sync(0xffffffffu, mx, off);
+        const double om = __shfl_xor_sync(0xffffffffu, mx, off);
         if (ov < bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-        mx = fmaxf(mx, om);
+        mx = fmax(mx, om);
     }
 }
 
-// named barriers of the kernel (id 0 is __syncthreads)
 // amp(slot): producers -> consumers, the amplitude table of the slot's candidates of this generation is written;
 // part(slot): consumers -> producers, the slot's partial sums of this generation are written; kBarProd: producers only.
 __device__ __forceinline__ int bar_amp(int slot) { return slot ? 4 : 1; }
@@ -270,9 +293,9 @@ __global__ void __launch_bounds__(kTcThreads, 1) pt_tc_kernel(const BlockParams 
     auto popA_of = [&](int s) { return reinterpret_cast<double*>(slot(s) + L.s_popA); };
     auto popT_of = [&](int s) { return reinterpret_cast<double*>(slot(s) + L.s_popT); };
     auto box_of = [&](int s) { return reinterpret_cast<double*>(slot(s) + L.s_box); };     // [6] bad box, [7] a1 fixed, +8 lo, +16 hi
-    auto fit_of = [&](int s) { return reinterpret_cast<float*>(slot(s) + L.s_fit); };
+    auto fit_of = [&](int s) { return reinterpret_cast<double*>(slot(s) + L.s_fit); };
     auto amp_of = [&](int s) { return reinterpret_cast<float*>(slot(s) + L.s_amp); };
-    auto part_of = [&](int s) { return reinterpret_cast<float*>(slot(s) + L.s_part); };
+    auto part_of = [&](int s) { return reinterpret_cast<double*>(slot(s) + L.s_part); };
     auto xs_of = [&](int s) { return reinterpret_cast<float*>(slot(s) + L.s_xs); };
 
     const int tid = threadIdx.x, nthr = blockDim.x;
@@ -314,9 +337,9 @@ __global__ void __launch_bounds__(kTcThreads, 1) pt_tc_kernel(const BlockParams 
     pr.db1 = tc::make_desc(smem_u32(opB) + 2 * tc::kBChunk, tc::kBChunk, 128);
     pr.pit = 0;
 
-    auto reported = [&](float v) -> double {       // F_cor - 1/pi of cor = -v for the correlation objective
-        if (OBJ == kObjCor) return 1.0 / (atan(-(double)v) + 0.5 * kPi) - 1.0 / kPi;
-        return (double)v;
+    auto reported = [&](double v) -> double {       // F_cor - 1/pi of cor = -v for the correlation objective
+        if (OBJ == kObjCor) return 1.0 / (atan(-v) + 0.5 * kPi) - 1.0 / kPi;
+        return v;
     };
     const int passes = (MODE == kModeFit) ? p.G + 1 : 1;
     const long long item_end = p.count ? min(p.B, p.blk0 + (long long)*p.count) : p.B;
@@ -387,7 +410,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) pt_tc_kernel(const BlockParams 
                     const bool a1z = (OBJ == kObjChi2) && box_of(s)[7] != 0.0;
                     named_sync(bar_amp(s), kTcThreads);
                     const float na0 = amp[2 * cand], na1 = amp[2 * cand + 1];
-                    float sum;
+                    double sum;
                     if (OBJ == kObjCor) sum = tc_consumer_pass<kTcAmpCor>(cs, xs, p.N, nT, c0, off, na0, na1, dtf, Ldtf, tw0);
                     else if (a1z) sum = tc_consumer_pass<kTcAmpConst>(cs, xs, p.N, nT, c0, off, na0, na1, dtf, Ldtf, tw0);
                     else sum = tc_consumer_pass<kTcAmpLinear>(cs, xs, p.N, nT, c0, off, na0, na1, dtf, Ldtf, tw0);
@@ -400,10 +423,10 @@ __global__ void __launch_bounds__(kTcThreads, 1) pt_tc_kernel(const BlockParams 
             const int i = tid - kTcConsumerWarps * 32;
             const bool active = i < p.NP;
             // sum of the four column groups' partials of member i, in fixed order; Eq. 5-6: the value minimised is -cor = (-a0) S
-            auto combined = [&](int s) -> float {
-                const float* part = part_of(s);
-                float v = ((part[i] + part[kTcMaxNP + i]) + part[2 * kTcMaxNP + i]) + part[3 * kTcMaxNP + i];
-                if (OBJ == kObjCor) v *= amp_of(s)[2 * i];
+            auto combined = [&](int s) -> double {
+                const double* part = part_of(s);
+                double v = ((part[i] + part[kTcMaxNP + i]) + part[2 * kTcMaxNP + i]) + part[3 * kTcMaxNP + i];
+                if (OBJ == kObjCor) v *= (double)amp_of(s)[2 * i];
                 return v;
             };
             // hand the candidate to the consumers (amplitude table), then emit the coefficient rows of all its tiles
@@ -439,12 +462,12 @@ __global__ void __launch_bounds__(kTcThreads, 1) pt_tc_kernel(const BlockParams 
                 for (int s = 0; s < na; ++s) {
                     double* popA = popA_of(s);
                     double* popT = popT_of(s);
-                    float* fit = fit_of(s);
+                    double* fit = fit_of(s);
                     const double* lo_s = box_of(s) + 8;
                     const double* hi_s = box_of(s) + 16;
                     named_sync(bar_part(s), kTcThreads);               // the slot's sums of generation g - 1 are complete
                     if (active) {
-                        const float v = combined(s);
+                        const double v = combined(s);
                         if (g == 1) {
                             fit[i] = v;
                             if (MODE == kModeFitness) p.fitness_out[blk_of[s] * (long long)p.NP + i] = (float)reported(v);
@@ -459,7 +482,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) pt_tc_kernel(const BlockParams 
                     const uint32_t bidx = bidx_of(s);
                     int ibest = 0;
                     if (p.strategy == kLocalToBest1 || p.strategy == kBest1Jitter) {
-                        float bv, mx;
+                        double bv, mx;
                         tc_warp_argmin(fit, p.NP, lane, bv, ibest, mx);
                     }
                     double th[D];
@@ -497,10 +520,10 @@ __global__ void __launch_bounds__(kTcThreads, 1) pt_tc_kernel(const BlockParams 
                 for (int s = 0; s < na; ++s) {
                     const long long blk = blk_of[s];
                     const double* popA = popA_of(s);
-                    const float* fit = fit_of(s);
+                    const double* fit = fit_of(s);
                     const double* box = box_of(s);
                     if (warp == kTcConsumerWarps) {
-                        float bv, mx;
+                        double bv, mx;
                         int bi;
                         tc_warp_argmin(fit, p.NP, lane, bv, bi, mx);
                         if (lane == 0) {
@@ -512,16 +535,16 @@ __global__ void __launch_bounds__(kTcThreads, 1) pt_tc_kernel(const BlockParams 
                                 const double w = box[16 + j] - box[8 + j];
                                 if (w > 0.0 && (v - box[8 + j] <= 1e-6 * w || box[16 + j] - v <= 1e-6 * w)) st |= 1u;
                             }
-                            const float braw = fit[bi];
+                            const double braw = fit[bi];
                             if (OBJ == kObjCor) {
                                 const double fb = reported(bv), fw = reported(mx);
                                 if (fw - fb > 1e-3 * fb) st |= 2u;
                                 p.best_rss[blk] = (float)reported(braw);
                             } else {
-                                if (mx - bv > 1e-3f * bv) st |= 2u;
-                                p.best_rss[blk] = braw;
+                                if (mx - bv > 1e-3 * bv) st |= 2u;
+                                p.best_rss[blk] = (float)braw;
                             }
-                            if (!(fabsf(braw) <= 3.0e38f)) st |= 8u;       // objective of the best member is not finite
+                            if (!(fabs(braw) <= 3.0e38)) st |= 8u;         // objective of the best member is not finite
                             if (box[6] != 0.0) st |= 16u;                  // the caller's box has lo > hi (or NaN) in some coordinate
                             p.status[blk] = st;
                         }

@@ -98,6 +98,8 @@ def lib():
     L.pt_doppler_products.restype = i32
     L.pt_track_host.argtypes = [p, i64, i32, f64, p, p, C.POINTER(DEConfig), f64, p, i32, p, p, p, p, p, p]
     L.pt_track_host.restype = i32
+    L.pt_host_cache_release.argtypes = []
+    L.pt_host_cache_release.restype = i32
     L.pt_de_draws.argtypes = [p, i64, i32, i32, f64, u64, p, p]
     L.pt_de_draws.restype = i32
     L.pt_init_population.argtypes = [p, p, p, i64, i32, i32, u64, p, p]
@@ -319,6 +321,11 @@ def pt_track_host(x, fs: float, lo, hi, cfg: DEConfig, los_scale: float = 0.0, b
     _check(rc, "pt_track_host")
     return {"best": best, "best_rss": best_rss, "status": status, "per_block": per_block, "total_phase": total,
             "intervals": outs}
+
+
+def pt_host_cache_release() -> None:
+    """Free the per-device memory pools and streams the *_host entry points keep between calls."""
+    _check(lib().pt_host_cache_release(), "pt_host_cache_release")
 
 
 def pt_track_auto_host(x, fs: float, cfg: DEConfig, acq: AcqConfig, retry: RetryConfig | None = None,

@@ -90,3 +90,18 @@ def test_inverted_box_sets_status_bit4_on_the_device_path_and_is_an_error_on_the
     cfg = pt.make_config(D=5, NP=60, generations=5, seed=5, t0=wl.t0)
     with pytest.raises(pt.PtError, match="lo > hi"):
         pt.pt_track_host(torch.from_numpy(wl.x), wl.fs, torch.from_numpy(lo), torch.from_numpy(hi), cfg)
+
+
+def test_host_entry_point_cache_can_be_released_and_recreated(pt):
+    """pt_track_host keeps a memory pool and a stream per device between calls (include/pt.h); releasing them must leave the
+    library usable and the results unchanged."""
+    wl = W.config0(cases=range(3))
+    cfg = pt.make_config(D=5, NP=60, generations=40, seed=5, t0=wl.t0)
+    args = (torch.from_numpy(wl.x), wl.fs, torch.from_numpy(wl.lo), torch.from_numpy(wl.hi), cfg, 0.0, [1])
+    a = pt.pt_track_host(*args)
+    b = pt.pt_track_host(*args)            # second call: served from the pool
+    pt.pt_host_cache_release()
+    pt.pt_host_cache_release()             # idempotent
+    c = pt.pt_track_host(*args)
+    for k in ("best", "best_rss", "status", "total_phase"):
+        assert torch.equal(a[k], b[k]) and torch.equal(a[k], c[k]), k
