@@ -54,6 +54,20 @@ def peak_probe(kind: int) -> float:
     return float(v.value)
 
 
+def sm_clock_probe(with_mma: bool) -> float:
+    """SM clock [MHz] a MUFU-bound kernel runs at, measured in-kernel (clock64 / globaltimer), without and with tcgen05.mma activity."""
+    import ctypes as C
+    from paper_1906_10598_b200 import build as _b
+    lib = C.CDLL(_b.build_probe())
+    lib.pt_bench_sm_clock.argtypes = [C.c_int32, C.c_void_p]
+    lib.pt_bench_sm_clock.restype = C.c_int32
+    v = C.c_double(0.0)
+    rc = lib.pt_bench_sm_clock(1 if with_mma else 0, C.byref(v))
+    if rc != 0:
+        raise RuntimeError("pt_bench_sm_clock failed (%d)" % rc)
+    return float(v.value)
+
+
 def algorithmic_traffic(wl, quant_bits: int = 0) -> float:
     """Bytes one step must move through HBM: every sample once, the boxes, and the per-block outputs."""
     D = wl.de["D"]
@@ -549,6 +563,10 @@ def main():
     try:
         roofline["measured_mufu_peak"] = peak_probe(1) / 1e12
         roofline["measured_ffma_peak_tflops"] = 2 * peak_probe(0) / 1e12
+        # the clock a kernel really runs at (in-kernel clock64 / globaltimer): tensor-core activity lowers it, nvidia-smi does not show it
+        roofline["sm_mhz_in_kernel"] = {"no_tensor_activity": sm_clock_probe(False), "with_tcgen05_mma": sm_clock_probe(True)}
+        if plan["threads"] == 640:
+            roofline["frac_at_in_kernel_clock"] = achieved / (SM_COUNT * XU_LANES_PER_SM * roofline["sm_mhz_in_kernel"]["with_tcgen05_mma"] * 1e6)
     except Exception as exc:  # diagnostics only
         roofline["probe_error"] = str(exc)
 

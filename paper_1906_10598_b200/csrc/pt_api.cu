@@ -108,9 +108,12 @@ static void choose_warp_grid(int warps, int groups, int nch, int* Wg, int* Ws) {
 }
 
 // Which evaluation kernel fits a block: pt_block_kernel (phase on the FP32 pipe) or pt_tc_kernel (phase on the tensor cores).
-// Automatic choice = whichever measured faster on the B200: the tensor-core kernel for D = 6 under chi^2 with
-// a population that fills at least three quarters of its 128 candidate lanes.  PT_KERNEL=tc / PT_KERNEL=classic in the
-// environment forces one of them where it applies (tests, A/B measurements); unset = automatic.
+// Automatic choice = whichever measured faster on the B200 (profiles/r2_kernel_choice.md): the tensor-core
+// kernel under chi^2 with a population that fills at least three quarters of its 128 candidate lanes when D = 6 (one more FP32
+// operation per sample-evaluation in pt_block_kernel, none here) or when the block is short (N <= 8192: two blocks per CTA hide
+// the DE step, which dominates short blocks).  A kernel that contains tcgen05.mma runs at 1845 instead of 1965 MHz on the B200,
+// which is why pt_block_kernel keeps the long D = 5 blocks.  PT_KERNEL=tc / PT_KERNEL=classic in the environment forces one of
+// them where it applies (tests, A/B measurements); unset = automatic.
 static int kernel_override() {
     const char* e = getenv("PT_KERNEL");
     if (!e || !*e) return 0;
@@ -118,12 +121,12 @@ static int kernel_override() {
     if (!strcmp(e, "classic")) return 2;
     return 0;
 }
-static bool want_tc(int NP, int D, int objective) {
+static bool want_tc(int N, int NP, int D, int objective) {
     if (NP > kTcMaxNP) return false;
     const int o = kernel_override();
     if (o == 1) return true;
     if (o == 2) return false;
-    return D == 6 && objective == kObjChi2 && NP >= 96;
+    return objective == kObjChi2 && NP >= 96 && (D == 6 || N <= 8192);
 }
 
 // sms / smem_optin are passed in so that the plan can also be computed without a device (defaults of B200).
@@ -160,7 +163,7 @@ static int make_plan(long long B, int N, int NP, int D, int sms, int smem_optin,
             }
         }
     }
-    if (want_tc(NP, D, objective)) {
+    if (want_tc(N, NP, D, objective)) {
         // one CTA of 640 threads per SM; shared memory holds the samples only, so the block must be resident
         for (int slots = 2; slots >= 1; --slots) {
             const TcSmemLayout L(N, NP, D, slots);

@@ -625,3 +625,35 @@ def test_full_size_config2_sampled_blocks(pt):
     o = _oracle_fit(sub, seed=1)
     assert abs(_wrap(g["best"][1234, 2] - o["best"][0, 2])) < PHI0_TOL
     assert abs(g["best"][1234, 3] - o["best"][0, 3]) < F_TOL
+
+
+def test_full_size_config3_sampled_blocks(pt):
+    """BASELINE config 3 at full size in bench.py's launch configuration (36000 x 10000 samples, NP = 128, D = 6, 1500
+    generations; the tensor-core kernel, two blocks per CTA, tail wave on clusters): properties on all blocks, sampled blocks
+    one by one with the oracle's objective, and one sampled block against the oracle's own DE fit."""
+    wl = W.config3()
+    g = _gpu_fit(pt, wl, seed=1)
+    assert np.all(np.isfinite(g["best"])) and np.all(np.isfinite(g["best_rss"]))
+    assert np.all(g["best"] >= wl.lo) and np.all(g["best"] <= wl.hi)
+    assert np.all((g["status"] & (2 | 8 | 16)) == 0)                  # collapsed, finite, boxes in order
+    # chi^2 at the optimum is the summed noise power (PAPER.md:151): (N - D) sigma^2 within 5 sigma on all blocks
+    z = (g["best_rss"] - (wl.N - 6) * wl.sigma**2) / (wl.sigma**2 * np.sqrt(2.0 * wl.N))
+    assert np.max(np.abs(z)) < 5.5 and abs(z.mean()) < 0.1
+    for k in range(0, 36000, 1500):
+        r_or = oracle.rss(wl.x[k], wl.fs, g["best"][k])
+        assert abs(g["best_rss"][k] - r_or) / r_or < FIT_REL_TOL
+        assert r_or <= oracle.rss(wl.x[k], wl.fs, wl.truth[k]) * (1 + 1e-9)
+    # Eq. 16-17: the 60-s integrated phase against the analytic phase advance; sigma of a block's increment from the
+    # Cramer-Rao bound of f (unfaded blocks; the fade around t = 1800 s is excluded from the bound, not from the sum)
+    pb, tot, iv = pt.pt_doppler_products(_cuda(g["best"]), wl.T, 0.0, [10, 100, 600])
+    phi60 = iv[2].cpu().numpy()[:, 0]
+    true60 = wl.meta["dphi_true"].reshape(60, 600).sum(axis=1)
+    sd_f = _crlb(wl.truth[100], wl.N, wl.fs, wl.sigma, 6)[3]
+    sd60 = np.sqrt(600.0) * 2 * np.pi * sd_f * wl.T
+    clear = np.ones(60, dtype=bool)
+    clear[27:33] = False                                               # 1620 .. 1980 s: the faded minutes
+    assert np.max(np.abs(phi60 - true60)[clear]) < 5.0 * sd60
+    sub = W.config3(blocks=[23456])
+    o = _oracle_fit(sub, seed=1)
+    assert abs(_wrap(g["best"][23456, 2] - o["best"][0, 2])) < PHI0_TOL
+    assert abs(g["best"][23456, 3] - o["best"][0, 3]) < F_TOL

@@ -199,7 +199,9 @@ def test_automatic_choice_takes_the_tensor_core_kernel_for_config3(pt):
     plan = pt.pt_fit_blocks_plan(36000, 10000, cfg)
     assert plan["threads"] == 640 and plan["cands_per_thread"] == 1
     cfg5 = pt.make_config(D=5, NP=128, generations=1000, t0=-0.5)
-    assert pt.pt_fit_blocks_plan(3600, 16000, cfg5)["threads"] == 512
+    assert pt.pt_fit_blocks_plan(3600, 16000, cfg5)["threads"] == 512          # long D = 5 blocks stay on the FP32-pipe kernel
+    assert pt.pt_fit_blocks_plan(1024, 4096, cfg5)["threads"] == 640           # short blocks: two per CTA on the tensor-core kernel
+    assert pt.pt_fit_blocks_plan(1024, 4096, pt.make_config(D=5, NP=64, generations=10, t0=-0.5))["threads"] != 640
 
 
 def test_classic_kernel_still_covers_d6(pt):
