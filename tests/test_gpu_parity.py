@@ -637,8 +637,14 @@ def test_full_size_config3_sampled_blocks(pt):
     assert np.all(g["best"] >= wl.lo) and np.all(g["best"] <= wl.hi)
     assert np.all((g["status"] & (2 | 8 | 16)) == 0)                  # collapsed, finite, boxes in order
     # chi^2 at the optimum is the summed noise power: (N - D) sigma^2 within 5 sigma on all blocks
+    # -- where the box leaves the optimum free.  The literal box is +-20 % of |theta|: where the true phi0 happens to
+    # be within ~0.1 rad of zero its box is narrower than the noise moves the least-squares phase (4.7 mrad at 10 dB), the fit is
+    # a CONSTRAINED optimum and its chi^2 is larger (measured: 4 of 36000 blocks with z = 5.9 .. 8.7, all with |phi0_true| < 0.02):
+    # there only the lower side is asserted.
     z = (g["best_rss"] - (wl.N - 6) * wl.sigma**2) / (wl.sigma**2 * np.sqrt(2.0 * wl.N))
-    assert np.max(np.abs(z)) < 5.5 and abs(z.mean()) < 0.1
+    free = np.abs(wl.truth[:, 2]) > 0.15
+    assert np.max(np.abs(z[free])) < 5.5 and abs(z[free].mean()) < 0.1
+    assert np.min(z) > -5.5 and np.mean(z > 5.5) < 1e-3
     for k in range(0, 36000, 1500):
         r_or = oracle.rss(wl.x[k], wl.fs, g["best"][k])
         assert abs(g["best_rss"][k] - r_or) / r_or < FIT_REL_TOL
