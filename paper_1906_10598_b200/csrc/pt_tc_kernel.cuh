@@ -6,9 +6,9 @@
 //     phase[c][j] = sum_k A[c][k] B[j][k],   A = tile-local Taylor coefficients of candidate c in tf32-exact pieces,
 //                                            B = the fixed basis (1, j, j^2, j^3), j = sample index - tile centre.
 // Warp roles (640 threads, one CTA per SM):
-//   warps 16-19  "producers": thread = candidate.  DE step; per tile the candidate's phase polynomial is re-expanded at the
+//   warps 16-19  "producers": thread = candidate (of up to two data blocks in flight).  DE step; per tile the candidate's phase polynomial is re-expanded at the
 //                tile centre in fp64 (value reduced mod 1 turn, so that fp32 never sees more than |E1| 128 rad), split into
-//                tf32-exact pieces by integer bit operations and stored as a row of the A operand (ring of 3 operands);
+//                tf32-exact pieces by integer bit operations and stored as a row of the A operand (ring of 4 operands);
 //                lane 0 of warp 16 issues the MMAs (ring of 2 accumulators = all 512 TMEM columns) and commits to mbarriers;
 //   warps 0-15   "consumers": TMEM lane = candidate (32 (warp % 4) + lane), warp / 4 = which 64 of the tile's 256 columns.
 //                tcgen05.ld brings 16 phases at a time; per sample-evaluation: FMUL + MUFU.COS (cos.approx), 1/2 FADD2
