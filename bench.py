@@ -412,8 +412,9 @@ def main():
                     help="feed packed samples of this many bits (Table 3 formats, pt_fit_blocks_q / pt_track_host_q)")
     ap.add_argument("--fix-a1", action="store_true", help="fix the amplitude slope at zero (a1 box [0, 0], PAPER.md:139)")
     ap.add_argument("--objective", default="chi2", choices=["chi2", "cor"], help="Eq. 4 (default) or Eq. 5-6")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "tc", "classic"],
-                    help="force the tensor-core (pt_tc_kernel) or the FP32-pipe (pt_block_kernel) evaluation kernel (PT_KERNEL hook)")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "run", "tc", "classic"],
+                    help="force the forward-difference (pt_run_kernel), tensor-core (pt_tc_kernel) or FP32-pipe Horner (pt_block_kernel) "
+                         "evaluation kernel (PT_KERNEL hook)")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="weak: every rank fits its own track (default); strong: ONE track split into contiguous block ranges over "
                          "the ranks (shard.fit_track_sharded), all-gather of the fitted parameters before the Doppler products")

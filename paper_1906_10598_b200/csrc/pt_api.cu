@@ -11,6 +11,7 @@
 #include "../../include/pt.h"
 #include "pt_de_kernel.cuh"
 #include "pt_tc_kernel.cuh"
+#include "pt_run_kernel.cuh"
 #include "pt_internal.h"
 
 namespace pt {
@@ -40,6 +41,7 @@ struct Plan {
     int K, NpadS;           // cluster path: CTAs per block, padded samples of the largest slice (K = 1: Npad)
     int tc;                 // 1: the tensor-core kernel (pt_tc_kernel.cuh) fits these blocks
     int tc_slots;           //    data blocks one of its CTAs fits at the same time (2 when shared memory allows)
+    int run;                // 1: the run-local kernel (pt_run_kernel.cuh) fits these blocks
 };
 
 // Per-device facts and per-device launch attributes, keyed by the CUDA device ordinal and guarded by one mutex: a process may
@@ -107,33 +109,85 @@ static void choose_warp_grid(int warps, int groups, int nch, int* Wg, int* Ws) {
     }
 }
 
-// Which evaluation kernel fits a block: pt_block_kernel (phase on the FP32 pipe) or pt_tc_kernel (phase on the tensor cores).
-// Automatic choice = whichever measured faster on the B200 (profiles/r2_kernel_choice.md): the tensor-core
-// kernel under chi^2 with a population that fills at least three quarters of its 128 candidate lanes when D = 6 (one more FP32
-// operation per sample-evaluation in pt_block_kernel, none here) or when the block is short (N <= 8192: two blocks per CTA hide
-// the DE step, which dominates short blocks).  A kernel that contains tcgen05.mma runs at 1845 instead of 1965 MHz on the B200,
-// which is why pt_block_kernel keeps the long D = 5 blocks.  PT_KERNEL=tc / PT_KERNEL=classic in the environment forces one of
-// them where it applies (tests, A/B measurements); unset = automatic.
+// Which evaluation kernel fits a block: pt_run_kernel (thread = candidate, phase by run-local Horner with immediate indices: the
+// default), pt_block_kernel (lanes own samples, phase relative to a reference array) or pt_tc_kernel (phase on the tensor cores).
+// Automatic choice = whichever measured fastest on the B200 (profiles/r2_kernel_choice.md): pt_run_kernel
+// everywhere.  PT_KERNEL=run / tc / classic in the environment forces one of them where it applies (tests, A/B measurements).
 static int kernel_override() {
     const char* e = getenv("PT_KERNEL");
     if (!e || !*e) return 0;
     if (!strcmp(e, "tc")) return 1;
     if (!strcmp(e, "classic")) return 2;
+    if (!strcmp(e, "run")) return 3;
     return 0;
 }
 static bool want_tc(int N, int NP, int D, int objective) {
+    (void)N; (void)D; (void)objective;
     if (NP > kTcMaxNP) return false;
+    return kernel_override() == 1;
+}
+static bool want_run() {
     const int o = kernel_override();
-    if (o == 1) return true;
-    if (o == 2) return false;
-    return objective == kObjChi2 && NP >= 96 && (D == 6 || N <= 8192);
+    return o == 0 || o == 3;
+}
+
+// Plan of pt_run_kernel: one CTA of 1024 threads per SM, or 2 x 512 / 4 x 256 when shared memory and the number of blocks allow (the
+// DE step of one CTA then overlaps with the evaluation of the others); with few blocks a cluster of K CTAs per block; blocks
+// larger than shared memory are streamed through a ring of 3 tiles.
+static int make_plan_run(long long B, int N, int NP, int D, int sms, int smem_optin, int force_K, Plan* pl) {
+    pl->sms = sms;
+    pl->tc = 0; pl->tc_slots = 1; pl->run = 1;
+    pl->C = 1; pl->NPpad = NP; pl->Wg = 1; pl->Ws = 1;
+    pl->Npad = (N + 3) & ~3;
+    pl->K = 1; pl->NpadS = pl->Npad; pl->TS = 0; pl->S = 0; pl->ws_bytes = 0; pl->resident = 1;
+    const int per_sm_total = smem_optin + 1024;   // 228 KB per SM, 1 KB reserved per resident CTA
+    const int quads = pl->Npad / 4;
+    {
+        // few blocks, many SMs: K = the largest power of two <= min(8, SMs / B) that leaves every CTA at least two runs of samples
+        int K = 1;
+        while (K * 2 <= 8 && (long long)B * (K * 2) <= sms && N / (K * 2) >= 2 * kRun) K *= 2;
+        if (force_K > 0) { K = force_K; while (K > 1 && quads / K < 1) --K; }
+        if (K > 1) {
+            const int NresMax = ((quads + K - 1) / K + 1) * 4;
+            const RunSmemLayout L(NresMax, NP, D, kRunMaxThreads, 0, 0, K);
+            if (L.total <= smem_optin) {
+                pl->threads = kRunMaxThreads; pl->ctas_per_sm = 1; pl->smem = L.total; pl->K = K; pl->NpadS = NresMax;
+                const long long want = (long long)(sms / K) * K;
+                pl->grid = (int)((long long)B * K < want ? (long long)B * K : want);
+                return 0;
+            }
+        }
+    }
+    for (int cps = 4; cps >= 1; cps >>= 1) {
+        if (cps > 1 && B <= (long long)sms * (cps / 2)) continue;   // not enough blocks to want that many CTAs
+        const int threads = kRunMaxThreads / cps;
+        const RunSmemLayout L(pl->Npad, NP, D, threads);
+        if (L.total > smem_optin) continue;
+        if ((long long)(L.total + 1024) * cps > per_sm_total) continue;
+        pl->threads = threads; pl->ctas_per_sm = cps; pl->smem = L.total;
+        const long long want = (long long)sms * cps;
+        pl->grid = (int)(B < want ? B : want);
+        return 0;
+    }
+    // streamed
+    pl->resident = 0;
+    for (int TS = 16384; TS >= 1024; TS >>= 1) {
+        const RunSmemLayout L(pl->Npad, NP, D, kRunMaxThreads, TS, 3);
+        if (L.total > smem_optin) continue;
+        pl->threads = kRunMaxThreads; pl->ctas_per_sm = 1; pl->smem = L.total; pl->TS = TS; pl->S = 3;
+        pl->grid = (int)(B < sms ? B : sms);
+        pl->ws_bytes = (size_t)pl->grid * pl->Npad * sizeof(float);      // aligned fp32 copies of unaligned / quantised rows
+        return 0;
+    }
+    return 1;
 }
 
 // sms / smem_optin are passed in so that the plan can also be computed without a device (defaults of B200).
 // force_K > 0 overrides the cluster-size choice (tests, tuning); 0 = automatic
 static int make_plan(long long B, int N, int NP, int D, int sms, int smem_optin, int force_K, Plan* pl, int objective = 0) {
+    if (want_run() && make_plan_run(B, N, NP, D, sms, smem_optin, force_K, pl) == 0) return 0;
     pl->sms = sms;
-    pl->tc = 0; pl->tc_slots = 1;
+    pl->tc = 0; pl->tc_slots = 1; pl->run = 0;
     pl->C = (NP % 8 == 0) ? 8 : 4;
     pl->NPpad = (NP + pl->C - 1) / pl->C * pl->C;
     pl->Npad = (N + kChunk - 1) / kChunk * kChunk;
@@ -335,14 +389,75 @@ static int dispatch_tc(const BlockParams& p, const Plan& pl, int D, int objectiv
     return D == 5 ? launch_tc_kernel<5, MODE, kObjChi2>(p, pl, st) : launch_tc_kernel<6, MODE, kObjChi2>(p, pl, st);
 }
 
+// ---- pt_run_kernel ----
+template <int D, int MODE, bool STREAM, int OBJ>
+static int run_configure_smem(const Plan& pl) {
+    static int configured_smem[kMaxDevices];
+    int dev = 0;
+    if (check_cuda(cudaGetDevice(&dev), "cudaGetDevice")) return PT_ERR_CUDA;
+    if (dev < 0 || dev >= kMaxDevices) { set_error("device ordinal %d beyond the compiled limit %d", dev, kMaxDevices); return PT_ERR_CUDA; }
+    std::lock_guard<std::mutex> lock(g_dev_mutex);
+    if (pl.smem > configured_smem[dev]) {
+        if (check_cuda(cudaFuncSetAttribute(pt_run_kernel<D, MODE, STREAM, OBJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem), "cudaFuncSetAttribute"))
+            return PT_ERR_CUDA;
+        configured_smem[dev] = pl.smem;
+    }
+    return PT_OK;
+}
+
+template <int D, int MODE, bool STREAM, int OBJ>
+static int run_max_resident_clusters(const Plan& pl) {
+    if (run_configure_smem<D, MODE, STREAM, OBJ>(pl)) return 0;
+    cudaLaunchConfig_t cfg;
+    cudaLaunchAttribute attr[1];
+    cluster_launch_config(pl, pl.K, nullptr, &cfg, attr);
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, pt_run_kernel<D, MODE, STREAM, OBJ>, &cfg) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return 0;
+    }
+    return n;
+}
+
+template <int D, int MODE, bool STREAM, int OBJ>
+static int launch_run_kernel(const BlockParams& p, const Plan& pl, cudaStream_t st) {
+    if (run_configure_smem<D, MODE, STREAM, OBJ>(pl)) return PT_ERR_CUDA;
+    if (pl.K > 1) {
+        int grid = pl.grid;
+        const int max_clusters = run_max_resident_clusters<D, MODE, STREAM, OBJ>(pl);
+        if (max_clusters > 0 && grid > max_clusters * pl.K) grid = max_clusters * pl.K;   // persistent: resident clusters only
+        cudaLaunchConfig_t cfg;
+        cudaLaunchAttribute attr[1];
+        cluster_launch_config(pl, grid, st, &cfg, attr);
+        if (check_cuda(cudaLaunchKernelEx(&cfg, pt_run_kernel<D, MODE, STREAM, OBJ>, p), "pt_run_kernel cluster launch")) return PT_ERR_CUDA;
+        return PT_OK;
+    }
+    pt_run_kernel<D, MODE, STREAM, OBJ><<<pl.grid, pl.threads, pl.smem, st>>>(p);
+    if (check_cuda(cudaGetLastError(), "pt_run_kernel launch")) return PT_ERR_CUDA;
+    return PT_OK;
+}
+
+template <int MODE, bool STREAM>
+static int dispatch_run2(const BlockParams& p, const Plan& pl, int D, int objective, cudaStream_t st) {
+    if (objective == kObjCor) return D == 5 ? launch_run_kernel<5, MODE, STREAM, kObjCor>(p, pl, st) : launch_run_kernel<6, MODE, STREAM, kObjCor>(p, pl, st);
+    return D == 5 ? launch_run_kernel<5, MODE, STREAM, kObjChi2>(p, pl, st) : launch_run_kernel<6, MODE, STREAM, kObjChi2>(p, pl, st);
+}
+
+template <int MODE>
+static int dispatch_run(const BlockParams& p, const Plan& pl, int D, int objective, cudaStream_t st) {
+    return pl.S > 0 ? dispatch_run2<MODE, true>(p, pl, D, objective, st) : dispatch_run2<MODE, false>(p, pl, D, objective, st);
+}
+
 template <int MODE>
 static int dispatch(const BlockParams& p, const Plan& pl, int D, int objective, cudaStream_t st) {
+    if (pl.run) return dispatch_run<MODE>(p, pl, D, objective, st);
     if (pl.tc) return dispatch_tc<MODE>(p, pl, D, objective, st);
     return pl.S > 0 ? dispatch2<MODE, true>(p, pl, D, objective, st) : dispatch2<MODE, false>(p, pl, D, objective, st);
 }
 
 // the shared-memory footprint, register count and launch bounds do not depend on the objective
 static int fit_max_resident_clusters(const Plan& pl, int D) {
+    if (pl.run) return D == 5 ? run_max_resident_clusters<5, kModeFit, false, kObjChi2>(pl) : run_max_resident_clusters<6, kModeFit, false, kObjChi2>(pl);
     if (pl.C == 8) return D == 5 ? max_resident_clusters<8, 5, kModeFit, false, kObjChi2>(pl) : max_resident_clusters<8, 6, kModeFit, false, kObjChi2>(pl);
     return D == 5 ? max_resident_clusters<4, 5, kModeFit, false, kObjChi2>(pl) : max_resident_clusters<4, 6, kModeFit, false, kObjChi2>(pl);
 }
@@ -352,8 +467,9 @@ static int fit_max_resident_clusters(const Plan& pl, int D) {
 // CTAs shares each block, so the tail costs 1/K of a wave.  K is lowered until `rem` clusters are resident at once.
 // Returns the number of tail blocks (0: single launch) and their plan.
 static long long plan_tail(long long B, int N, int NP, int D, const Plan& pl, Plan* tail) {
-    if (force_cluster() != 0 || pl.K != 1 || pl.S != 0 || pl.ctas_per_sm != 1 || B <= pl.sms) return 0;
-    const long long rem = B % pl.sms;
+    const long long slots = (long long)pl.sms * pl.ctas_per_sm;
+    if (force_cluster() != 0 || pl.K != 1 || pl.S != 0 || (pl.ctas_per_sm != 1 && !pl.run) || B <= slots) return 0;
+    const long long rem = B % slots;
     if (rem == 0 || rem * 2 > pl.sms) return 0;
     int sms = 0, smem_optin = 0;
     if (device_info(&sms, &smem_optin)) return 0;
@@ -369,6 +485,7 @@ static long long plan_tail(long long B, int N, int NP, int D, const Plan& pl, Pl
 static int attach_workspace(BlockParams* p, const Plan& pl, void* workspace, size_t workspace_bytes) {
     p->TS = pl.TS; p->S = pl.S;
     p->K = pl.K; p->NpadS = pl.NpadS; p->tc_slots = pl.tc_slots;
+    if (pl.run) { p->Npad = pl.Npad; p->NPpad = pl.NPpad; }
     if (pl.S == 0) return PT_OK;
     if (!workspace || workspace_bytes < pl.ws_bytes) {
         set_error("streamed path (N = %d does not fit in shared memory) needs %zu bytes of workspace, got %zu", p->N, pl.ws_bytes,
@@ -377,7 +494,7 @@ static int attach_workspace(BlockParams* p, const Plan& pl, void* workspace, siz
     }
     if (reinterpret_cast<uintptr_t>(workspace) % 16) { set_error("workspace must be 16-byte aligned"); return PT_ERR_INVALID_ARG; }
     p->ws_wref = reinterpret_cast<float*>(workspace);
-    p->ws_x = p->ws_wref + (size_t)pl.grid * pl.Npad;
+    p->ws_x = pl.run ? p->ws_wref : p->ws_wref + (size_t)pl.grid * pl.Npad;      // pt_run_kernel has no reference-phase rows
     return PT_OK;
 }
 

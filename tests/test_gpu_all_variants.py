@@ -54,21 +54,38 @@ def _fit(pt, wl, NP, G, D=5, strategy=1, objective=0, env=None, quant=None):
 
 
 SMALL = lambda: W.single_tone_blocks(range(6), 1024, 1024.0, config=4, f_range=(20, 60))
+CUBIC = lambda: W.single_tone_blocks(range(3), 1024, 1024.0, config=4, f_range=(20, 60))     # fs = 1 kHz: the cubic term matters inside a run
 CASES = {
-    "classic resident D5, automatic clusters": (SMALL, dict(NP=16, G=3), dict(cluster=lambda k: k >= 2)),
-    "classic resident D5, single CTA": (SMALL, dict(NP=16, G=3, env={"PT_CLUSTER": "1"}), dict(threads=512, cluster=1)),
-    "classic cluster of 8": (lambda: W.single_tone_blocks(range(2), 4096, 4096.0, config=4), dict(NP=16, G=2, env={"PT_CLUSTER": "8"}), dict(cluster=8)),
+    # ---- pt_run_kernel (the automatic choice) ----
+    "run resident D5, automatic clusters": (SMALL, dict(NP=16, G=3), dict(threads=1024, cluster=lambda k: k >= 2)),
+    "run resident D5, single CTA": (SMALL, dict(NP=16, G=3, env={"PT_CLUSTER": "1"}), dict(threads=1024, cluster=1)),
+    "run cluster of 8": (lambda: W.single_tone_blocks(range(2), 4096, 4096.0, config=4), dict(NP=16, G=2, env={"PT_CLUSTER": "8"}), dict(threads=1024, cluster=8)),
+    "run cluster of 3, N % 4 == 2": (lambda: W.single_tone_blocks(range(2), 4098, 4098.0, config=4), dict(NP=16, G=2, env={"PT_CLUSTER": "3"}), dict(cluster=3)),
+    "run strategy 3 + correlation": (SMALL, dict(NP=16, G=3, strategy=3, objective=1, env={"PT_CLUSTER": "1"}), dict(cluster=1)),
+    "run resident D6 (cubic folded into the run's second derivative)": (lambda: W.config3(blocks=[10, 11, 12]), dict(NP=16, G=2, D=6, env={"PT_CLUSTER": "1"}), dict(threads=1024)),
+    "run more members than threads": (SMALL, dict(NP=1024, G=1, env={"PT_CLUSTER": "1"}), dict(threads=1024)),
+    "run 4 CTAs per SM + cluster tail": (lambda: W.single_tone_blocks(range(600), 512, 512.0, config=4, f_range=(20, 60)),
+                                         dict(NP=16, G=2), dict(threads=256, ctas_per_sm=4, tail_cluster=lambda k: k >= 2)),
+    "run 2 CTAs per SM": (lambda: W.single_tone_blocks(range(160), 512, 512.0, config=4, f_range=(20, 60)), dict(NP=8, G=2), dict(threads=512, ctas_per_sm=2)),
+    "run streamed ring": (lambda: W.single_tone_blocks(range(2), 65536, 65536.0, config=4), dict(NP=16, G=1, env={"PT_CLUSTER": "1"}), dict(resident=0, threads=1024)),
+    "run streamed ring, quantised 4 bit": (lambda: W.single_tone_blocks(range(2), 65536, 65536.0, config=4), dict(NP=16, G=1, quant=4, env={"PT_CLUSTER": "1"}), dict(resident=0)),
+    "run quantised 2 bit": (SMALL, dict(NP=16, G=2, quant=2, env={"PT_CLUSTER": "1"}), dict(threads=1024)),
+    # ---- pt_block_kernel (PT_KERNEL=classic) ----
+    "classic resident D5, automatic clusters": (SMALL, dict(NP=16, G=3, env={"PT_KERNEL": "classic"}), dict(threads=512, cluster=lambda k: k >= 2)),
+    "classic resident D5, single CTA": (SMALL, dict(NP=16, G=3, env={"PT_CLUSTER": "1", "PT_KERNEL": "classic"}), dict(threads=512, cluster=1)),
+    "classic cluster of 8": (lambda: W.single_tone_blocks(range(2), 4096, 4096.0, config=4), dict(NP=16, G=2, env={"PT_CLUSTER": "8", "PT_KERNEL": "classic"}), dict(threads=512, cluster=8)),
     "classic strategy 3 + correlation": (SMALL, dict(NP=16, G=3, strategy=3, objective=1, env={"PT_CLUSTER": "1", "PT_KERNEL": "classic"}), dict(cluster=1)),
     "classic resident D6": (lambda: W.config3(blocks=[10, 11, 12]), dict(NP=16, G=2, D=6, env={"PT_CLUSTER": "1", "PT_KERNEL": "classic"}), dict(threads=512)),
+    "classic persistent loop + tail launch": (lambda: W.single_tone_blocks(range(158), 512, 512.0, config=4, f_range=(20, 60)),
+                                              dict(NP=8, G=2, env={"PT_KERNEL": "classic"}), dict(resident=1)),
+    "classic streamed ring": (lambda: W.single_tone_blocks(range(2), 65536, 65536.0, config=4), dict(NP=16, G=1, env={"PT_CLUSTER": "1", "PT_KERNEL": "classic"}), dict(resident=0, threads=512)),
+    "classic quantised 2 bit": (SMALL, dict(NP=16, G=2, quant=2, env={"PT_CLUSTER": "1", "PT_KERNEL": "classic"}), dict(threads=512)),
+    # ---- pt_tc_kernel (PT_KERNEL=tc) ----
     "tensor-core D6, one block per CTA": (lambda: W.config3(blocks=[10, 11, 12]), dict(NP=32, G=2, D=6, env={"PT_CLUSTER": "1", "PT_KERNEL": "tc"}), dict(threads=640)),
     "tensor-core D5, two blocks per CTA + cluster tail": (lambda: W.single_tone_blocks(range(310), 512, 512.0, config=4, f_range=(20, 60)),
                                                           dict(NP=16, G=2, env={"PT_KERNEL": "tc"}), dict(threads=640, tail_cluster=lambda k: k >= 2)),
     "tensor-core quantised 8 bit": (SMALL, dict(NP=16, G=2, quant=8, env={"PT_CLUSTER": "1", "PT_KERNEL": "tc"}), dict(threads=640)),
     "tensor-core correlation objective": (SMALL, dict(NP=16, G=2, objective=1, env={"PT_CLUSTER": "1", "PT_KERNEL": "tc"}), dict(threads=640)),
-    "classic persistent loop + tail launch": (lambda: W.single_tone_blocks(range(158), 512, 512.0, config=4, f_range=(20, 60)),
-                                              dict(NP=8, G=2, env={"PT_KERNEL": "classic"}), dict(resident=1)),
-    "classic streamed ring": (lambda: W.single_tone_blocks(range(2), 65536, 65536.0, config=4), dict(NP=16, G=1, env={"PT_CLUSTER": "1"}), dict(resident=0)),
-    "classic quantised 2 bit": (SMALL, dict(NP=16, G=2, quant=2, env={"PT_CLUSTER": "1", "PT_KERNEL": "classic"}), dict(threads=512)),
 }
 
 

@@ -1,0 +1,233 @@
+"""GPU parity of the three evaluation kernels against the fp64 oracle, through the C ABI, on the same inputs:
+  run      pt_run_kernel   (the automatic choice: thread = candidate, phase by run-local Horner)
+  classic  pt_block_kernel (lanes own samples, phase relative to a reference array)
+  tc       pt_tc_kernel    (phase on the tensor cores; its own file: test_gpu_tc.py)
+PT_KERNEL is the library's documented hook that forces one of them (include/pt.h).  The rest of the GPU suite runs the automatic
+choice; this file keeps pt_block_kernel covered at the same bars and checks what is specific to pt_run_kernel: the cubic loop,
+the per-block switch between the two D = 6 loops, short last runs, several CTAs per SM, members spread over several slices.
+Bars are north_star's: fitness <= 1e-4 relative on identical populations, |dphi0| < 5 mrad, |df| < 1e-3 Hz."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1906_10598_b200 import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+FIT_REL_TOL, PHI0_TOL, F_TOL = 1e-4, 5e-3, 1e-3
+
+
+@pytest.fixture(scope="module")
+def pt():
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu-marked tests need a CUDA device; there is no CPU fallback")
+    from paper_1906_10598_b200 import pt as _pt
+    _pt.lib()
+    return _pt
+
+
+class _env:
+    def __init__(self, kernel="", cluster=""):
+        self.want = {"PT_KERNEL": kernel, "PT_CLUSTER": cluster}
+
+    def __enter__(self):
+        self.old = {k: os.environ.get(k) for k in self.want}
+        for k, v in self.want.items():
+            if v:
+                os.environ[k] = v
+            else:
+                os.environ.pop(k, None)
+
+    def __exit__(self, *a):
+        for k, v in self.old.items():
+            if v is None:
+                os.environ.pop(k, None)
+            else:
+                os.environ[k] = v
+
+
+def _cuda(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _wrap(d):
+    return (np.asarray(d) + np.pi) % (2 * np.pi) - np.pi
+
+
+def _population(wl, NP, seed, spread=1.0):
+    rng = np.random.default_rng(seed)
+    c, h = 0.5 * (wl.lo + wl.hi), 0.5 * (wl.hi - wl.lo) * spread
+    return (c[:, None, :] + h[:, None, :] * rng.uniform(-1, 1, (wl.B, NP, wl.lo.shape[1]))).astype(np.float32)
+
+
+def _with_fddot(wl, half_width):
+    """A D = 5 single-tone workload seen as D = 6: truth fddot = 0, box +- half_width [Hz/s^2]."""
+    z = np.zeros((wl.B, 1))
+    wl.truth = np.hstack([wl.truth, z])
+    wl.lo = np.hstack([wl.lo, z - half_width])
+    wl.hi = np.hstack([wl.hi, z + half_width])
+    wl.de = dict(wl.de, D=6)
+    return wl
+
+
+def _fit(pt, wl, *, NP, generations, seed, D=None, want_pop=False, F=0.5, CR=0.9):
+    cfg = pt.make_config(D=D or wl.lo.shape[1], NP=NP, generations=generations, F=F, CR=CR, seed=seed, t0=wl.t0)
+    r = pt.pt_fit_blocks(_cuda(wl.x), wl.fs, _cuda(wl.lo), _cuda(wl.hi), cfg, block_index=_cuda(wl.block_index.astype(np.int32)),
+                         want_pop=want_pop)
+    torch.cuda.synchronize()
+    return {k: v.cpu().numpy() for k, v in r.items()}
+
+
+# ----------------------------------------------------------------------------------------------
+# fitness on identical populations, every kernel
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", ["run", "classic"])
+@pytest.mark.parametrize("make,NP", [(lambda: W.config0(cases=range(5)), 60), (lambda: W.config1(blocks=[0, 59]), 100),
+                                     (lambda: W.config2(blocks=[0, 1800, 3599]), 128), (lambda: W.config3(blocks=[0, 17950, 35999]), 128)])
+def test_fitness_parity_configs(pt, kernel, make, NP):
+    wl = make()
+    for spread, seed in ((1.0, NP), (1e-4, NP + 1)):          # random in the box; collapsed around its centre
+        pop = _population(wl, NP, seed, spread)
+        ref = oracle.fitness(wl.x, wl.fs, pop)
+        for cluster in ("1", ""):
+            with _env(kernel, cluster):
+                got = pt.pt_fitness(_cuda(wl.x), wl.fs, _cuda(pop)).cpu().numpy()
+            rel = np.abs(got - ref) / ref
+            print("\n[%s fitness %s NP=%d spread %g cluster %r] max rel err %.2e" % (kernel, wl.name, NP, spread, cluster, rel.max()))
+            assert rel.max() < FIT_REL_TOL
+
+
+@pytest.mark.parametrize("N,NP", [(8, 4), (10, 5), (126, 7), (130, 7), (258, 33), (1030, 13), (4094, 128), (16384, 512), (2048, 1024)])
+def test_run_kernel_ragged_sizes_and_high_rates(pt, N, NP):
+    """Carrier at 0.05 ... 0.2 cycles per sample (|E1| up to 1.5 rad per sample: the largest fp32 phases the run-local polynomial
+    sees), N not a multiple of the 128-sample run or of 4, short last runs, members over several slices / more members than
+    threads; with and without clusters."""
+    wl = W.single_tone_blocks(range(5), N, float(N), config=4, f_range=(0.05 * N, 0.2 * N))
+    pop = _population(wl, NP, N)
+    ref = oracle.fitness(wl.x, wl.fs, pop)
+    for cluster in ("1", "", "3"):
+        with _env("run", cluster):
+            got = pt.pt_fitness(_cuda(wl.x), wl.fs, _cuda(pop)).cpu().numpy()
+        assert np.max(np.abs(got - ref) / ref) < FIT_REL_TOL, cluster
+
+
+# ----------------------------------------------------------------------------------------------
+# D = 6: the two loops of pt_run_kernel and the switch between them
+# ----------------------------------------------------------------------------------------------
+def test_run_kernel_cubic_loop(pt):
+    """fs = 4096 Hz and a +-200 Hz/s^2 box: the cubic term moves the phase by up to 8e-4 rad inside a 128-sample run, so the block
+    takes the loop that carries E3 (one more FFMA2 per pair); fitness against the oracle, random and collapsed populations."""
+    wl = _with_fddot(W.single_tone_blocks(range(4), 4096, 4096.0, config=4, f_range=(200.0, 800.0)), 200.0)
+    for spread in (1.0, 1e-3):
+        pop = _population(wl, 64, 7, spread)
+        ref = oracle.fitness(wl.x, wl.fs, pop)
+        for cluster in ("1", ""):
+            with _env("run", cluster):
+                got = pt.pt_fitness(_cuda(wl.x), wl.fs, _cuda(pop)).cpu().numpy()
+            assert np.max(np.abs(got - ref) / ref) < FIT_REL_TOL
+
+
+@pytest.mark.parametrize("half_width", [0.0, 1e-3, 3e-3, 1e-2, 1.0])
+def test_run_kernel_d6_loop_switch_is_invisible(pt, half_width):
+    """The per-block switch (cubic term inside a run below / above 1e-7 rad over the whole box) sits near a +-4e-3 Hz/s^2 box at
+    fs = 4096 Hz.  Boxes on both sides of it: on a collapsed population the objective agrees with the oracle to 5e-6 either way
+    (the dropped term is <= 1e-7 rad)."""
+    wl = _with_fddot(W.single_tone_blocks(range(3), 4096, 4096.0, config=4, f_range=(200.0, 800.0)), half_width)
+    pop = _population(wl, 32, 11, 1e-3)
+    ref = oracle.fitness(wl.x, wl.fs, pop)
+    with _env("run", "1"):
+        got = pt.pt_fitness(_cuda(wl.x), wl.fs, _cuda(pop)).cpu().numpy()
+    assert np.max(np.abs(got - ref) / ref) < 5e-6
+
+
+def test_run_kernel_d6_fit_config3_and_cubic(pt):
+    """Full D = 6 fits: config-3 blocks (cubic folded into the runs' second derivative) and a low-rate block with an observable
+    fddot (cubic loop), against the oracle's own fit."""
+    wl = W.config3(blocks=[100, 20000])
+    with _env("run", "1"):
+        g = _fit(pt, wl, NP=128, generations=1500, seed=4)
+    o = oracle.fit_blocks(wl.x, wl.fs, wl.lo, wl.hi, NP=128, generations=1500, seed=4, block_index=wl.block_index)
+    assert np.max(np.abs(g["best_rss"] - o["best_rss"]) / o["best_rss"]) < FIT_REL_TOL
+    assert np.max(np.abs(_wrap(g["best"][:, 2] - o["best"][:, 2]))) < PHI0_TOL
+    assert np.max(np.abs(g["best"][:, 3] - o["best"][:, 3])) < F_TOL
+    wl = _with_fddot(W.single_tone_blocks(range(3), 4096, 4096.0, config=4, f_range=(200.0, 800.0)), 50.0)
+    with _env("run", "1"):
+        g = _fit(pt, wl, NP=96, generations=600, seed=5)
+    o = oracle.fit_blocks(wl.x, wl.fs, wl.lo, wl.hi, NP=96, generations=600, seed=5, block_index=wl.block_index)
+    ok = np.abs(g["best_rss"] - o["best_rss"]) / o["best_rss"] < FIT_REL_TOL
+    assert ok.sum() >= 2, (g["best_rss"], o["best_rss"])
+    assert np.max(np.abs(_wrap(g["best"][ok, 2] - o["best"][ok, 2]))) < PHI0_TOL
+    assert np.max(np.abs(g["best"][ok, 3] - o["best"][ok, 3])) < F_TOL
+    for k in range(wl.B):       # every result is valid: its RSS is the oracle's objective at its own parameters
+        v = oracle.rss(wl.x[k], wl.fs, g["best"][k])
+        assert abs(float(g["best_rss"][k]) - v) / v < FIT_REL_TOL
+
+
+# ----------------------------------------------------------------------------------------------
+# DE trajectories and full fits, run and classic
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", ["run", "classic"])
+def test_first_generations_follow_the_oracle(pt, kernel):
+    """Same seed, same blocks: after 4 generations the populations are the oracle's member by member except where a selection
+    fell inside the fp32 / fp64 difference of the two objective values (R18); the observed fraction is printed."""
+    for wl, NP in ((W.config2(blocks=[5, 1700]), 128), (W.config1(blocks=[3, 40]), 100), (W.config3(blocks=[7, 18000]), 128)):
+        with _env(kernel, "1"):
+            g = _fit(pt, wl, NP=NP, generations=4, seed=21, want_pop=True)
+        o = oracle.fit_blocks(wl.x, wl.fs, wl.lo, wl.hi, NP=NP, generations=4, seed=21, block_index=wl.block_index, want_pop=True)
+        same = np.all(g["final_pop"] == o["final_pop"].astype(np.float32), axis=-1)
+        print("\n[%s trajectory %s] identical members after 4 generations: %.4f" % (kernel, wl.name, same.mean()))
+        assert same.mean() > 0.98
+        assert np.max(np.abs(g["final_fit"] - o["final_fit"]) / o["final_fit"]) < FIT_REL_TOL
+
+
+@pytest.mark.parametrize("kernel", ["run", "classic"])
+def test_full_fits_config0(pt, kernel):
+    wl = W.config0(cases=range(8))
+    with _env(kernel, "1"):
+        g = _fit(pt, wl, NP=60, generations=500, seed=2)
+    o = oracle.fit_blocks(wl.x, wl.fs, wl.lo, wl.hi, NP=60, generations=500, seed=2, block_index=wl.block_index)
+    assert np.max(np.abs(g["best_rss"] - o["best_rss"]) / o["best_rss"]) < FIT_REL_TOL
+    assert np.max(np.abs(_wrap(g["best"][:, 2] - o["best"][:, 2]))) < PHI0_TOL
+    assert np.max(np.abs(g["best"][:, 3] - o["best"][:, 3])) < F_TOL
+    assert np.array_equal(g["status"] & 3, o["status"] & 3)
+
+
+def test_kernels_agree_with_each_other(pt):
+    """run, classic and tc on the same 40 config-2 blocks: the fitted phase and frequency of every block agree at the parity bars
+    (the three kernels differ only in fp32 rounding of the objective)."""
+    wl = W.config2(blocks=range(100, 140), generations=400)
+    res = {}
+    for kernel in ("run", "classic", "tc"):
+        with _env(kernel, "1"):
+            res[kernel] = _fit(pt, wl, NP=128, generations=400, seed=8)
+    for a, b in (("run", "classic"), ("run", "tc")):
+        ok = ((res[a]["status"] & 2) == 0) & ((res[b]["status"] & 2) == 0)
+        assert ok.sum() >= 36
+        assert np.max(np.abs(_wrap(res[a]["best"][ok, 2] - res[b]["best"][ok, 2]))) < PHI0_TOL
+        assert np.max(np.abs(res[a]["best"][ok, 3] - res[b]["best"][ok, 3])) < F_TOL
+
+
+# ----------------------------------------------------------------------------------------------
+# launch geometries of pt_run_kernel
+# ----------------------------------------------------------------------------------------------
+def test_run_kernel_results_do_not_depend_on_the_launch_geometry(pt):
+    """700 short blocks on 4 CTAs per SM (+ the cluster tail) against the same blocks fitted 37 at a time (one 1024-thread CTA per
+    block): Philox streams depend on the block index only and the objective is summed in fp64 across slices, so the first
+    generations are the same populations."""
+    wl = W.config4(1024, 32, B=700, generations=3)
+    cfg = pt.make_config(D=5, NP=32, generations=3, seed=12, t0=wl.t0)
+    plan = pt.pt_fit_blocks_plan(wl.B, wl.N, cfg)
+    assert plan["ctas_per_sm"] == 4 and plan["threads"] == 256, plan
+    a = _fit(pt, wl, NP=32, generations=3, seed=12, want_pop=True)
+    sub = list(range(0, 700, 19))
+    w2 = W.config4(1024, 32, B=700, generations=3)
+    w2.x, w2.lo, w2.hi, w2.truth, w2.block_index = wl.x[sub], wl.lo[sub], wl.hi[sub], wl.truth[sub], wl.block_index[sub]
+    with _env("run", "1"):
+        assert pt.pt_fit_blocks_plan(w2.B, w2.N, cfg)["threads"] == 1024
+        b = _fit(pt, w2, NP=32, generations=3, seed=12, want_pop=True)
+    same = np.all(a["final_pop"][sub] == b["final_pop"], axis=-1)
+    assert same.mean() > 0.995, same.mean()
+    assert np.max(np.abs(a["final_fit"][sub] - b["final_fit"]) / b["final_fit"]) < 1e-5

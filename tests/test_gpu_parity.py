@@ -163,15 +163,40 @@ def test_fitness_unaligned_rows_take_the_non_bulk_path(pt):
 # ----------------------------------------------------------------------------------------------
 # streamed path: blocks larger than shared memory (BASELINE config 4: 64 K and 256 K samples)
 # ----------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("N,NP,B", [(65536, 32, 3), (65536, 512, 2), (262144, 64, 2), (65536 + 130, 40, 2), (65536 + 132, 24, 2),
-                                    (70002, 16, 2), (30000, 12, 150), (32768, 1024, 1)])
-def test_fitness_streamed_blocks(pt, no_cluster, N, NP, B):
-    """Tiles of the block move through the shared-memory ring; partial last tile, partial last chunk, rows that are
-    not 16-byte aligned (N % 4 == 2: copied to the workspace first), more blocks than CTAs, largest population."""
-    cfg = pt.make_config(D=5, NP=NP, generations=1, t0=0.0)
-    assert pt.pt_fit_blocks_plan(B, N, cfg)["resident"] == 0
-    wl = W.single_tone_blocks(range(B), N, float(N), config=4, f_range=(50.0, 200.0))
-    assert _fitness_case(pt, wl, NP=NP, seed=N + NP) < FIT_REL_TOL
+class _forced_kernel:
+    """PT_KERNEL=run / classic / tc forces one of the evaluation kernels (include/pt.h); unset = the automatic choice."""
+
+    def __init__(self, which):
+        self.which = which
+
+    def __enter__(self):
+        import os
+        self.old = os.environ.get("PT_KERNEL")
+        if self.which:
+            os.environ["PT_KERNEL"] = self.which
+
+    def __exit__(self, *a):
+        import os
+        if self.old is None:
+            os.environ.pop("PT_KERNEL", None)
+        else:
+            os.environ["PT_KERNEL"] = self.old
+
+
+@pytest.mark.parametrize("kernel,N,NP,B", [
+    ("", 65536, 32, 3), ("", 65536, 512, 2), ("", 262144, 64, 2), ("", 65536 + 130, 40, 2), ("", 65536 + 132, 24, 2), ("", 70002, 16, 2),
+    ("", 60000, 12, 150), ("", 65536, 1024, 1), ("", 100000 + 2, 400, 1),
+    ("classic", 65536, 32, 3), ("classic", 65536 + 130, 40, 2), ("classic", 70002, 16, 2), ("classic", 30000, 12, 150),
+    ("classic", 32768, 1024, 1)])
+def test_fitness_streamed_blocks(pt, no_cluster, kernel, N, NP, B):
+    """Tiles of the block move through the shared-memory ring; partial last tile, partial last run / chunk, rows that are
+    not 16-byte aligned (N % 4 == 2: copied to the workspace first), more blocks than CTAs, more members than threads; both
+    kernels that have a streamed path (the automatic pt_run_kernel and pt_block_kernel)."""
+    with _forced_kernel(kernel):
+        cfg = pt.make_config(D=5, NP=NP, generations=1, t0=0.0)
+        assert pt.pt_fit_blocks_plan(B, N, cfg)["resident"] == 0
+        wl = W.single_tone_blocks(range(B), N, float(N), config=4, f_range=(50.0, 200.0))
+        assert _fitness_case(pt, wl, NP=NP, seed=N + NP) < FIT_REL_TOL
 
 
 def test_fit_streamed_trajectory_and_full_fit(pt, no_cluster):
@@ -201,7 +226,9 @@ def test_streamed_needs_workspace(pt, no_cluster):
     L = pt.lib()
     cfg = pt.make_config(D=5, NP=32, generations=1, t0=-0.5)
     need = L.pt_fit_blocks_workspace_bytes(2, 65536, C.byref(cfg))
-    assert need == 2 * 65536 * 4 * 2
+    assert need == 2 * 65536 * 4          # pt_run_kernel: one fp32 row per CTA (aligned copy of an unaligned / quantised block)
+    with _forced_kernel("classic"):
+        assert L.pt_fit_blocks_workspace_bytes(2, 65536, C.byref(cfg)) == 2 * 65536 * 4 * 2      # + the reference-phase row
     x = torch.zeros((2, 65536), dtype=torch.float32, device="cuda")
     box = torch.zeros((2, 5), dtype=torch.float64, device="cuda")
     best = torch.empty((2, 5), dtype=torch.float64, device="cuda")
@@ -280,19 +307,17 @@ def test_fit_cluster_persistent_loop_and_single_cta_agree(pt):
 
 
 def test_tail_wave_is_fitted_by_clusters_and_matches_the_single_launch(pt):
-    """B = SMs + a few blocks: the full wave runs on single CTAs, the remainder on clusters (second launch).  Same
+    """B = one full wave + a few blocks: the full wave runs on single CTAs, the remainder on clusters (second launch).  Same
     blocks with PT_CLUSTER=1 (one launch, no clusters): the Philox streams depend on the block index only, so the
     first generations are identical populations and the outputs land in the right rows."""
     sms = torch.cuda.get_device_properties(0).multi_processor_count
-    B = sms + 5
+    cfg = pt.make_config(D=5, NP=32, generations=2, seed=6, t0=-0.5)
+    cps = pt.pt_fit_blocks_plan(100 * sms, 2048, cfg)["ctas_per_sm"]          # several CTAs per SM for blocks this short
+    B = sms * cps + 5
     wl = W.config4(2048, 32, B=B, generations=2)
     cfg = pt.make_config(D=5, NP=32, generations=2, seed=6, t0=wl.t0)
     plan = pt.pt_fit_blocks_plan(B, 2048, cfg)
-    if plan["ctas_per_sm"] != 1:
-        # small blocks run several CTAs per SM and keep the single launch; use blocks that fill an SM
-        wl = W.config4(16384, 32, B=B, generations=2)
-        cfg = pt.make_config(D=5, NP=32, generations=2, seed=6, t0=wl.t0)
-        plan = pt.pt_fit_blocks_plan(B, 16384, cfg)
+    assert plan["ctas_per_sm"] == cps and plan["grid"] == sms * cps, plan
     assert plan["cluster"] == 1 and plan["tail_cluster"] == 8, plan
     a = _gpu_fit(pt, wl, generations=2, seed=6, want_pop=True)
     with _forced_cluster(1):

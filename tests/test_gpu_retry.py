@@ -118,31 +118,32 @@ def test_invalid_retry_arguments(pt):
 
 
 def test_re_search_over_a_selection_larger_than_one_wave(pt):
-    """160 doubtful blocks of 480: the selection list spans a full wave of single CTAs plus a tail wave on clusters
-    (pt_fit_blocks_plan's tail_cluster), each work item writing to its own block's rows."""
-    wl = W.config2(blocks=range(480), generations=120, NP=32)
+    """320 doubtful blocks of 960: the selection list is longer than one wave of the persistent grid (2 CTAs per SM), each work
+    item writing to its own block's rows."""
+    NB = 960
+    wl = W.config2(blocks=range(NB), generations=120, NP=32)
     cfg = pt.make_config(D=5, NP=32, generations=120, seed=4, t0=wl.t0)
     xd = _cuda(wl.x)
     ref = pt.pt_fit_blocks(xd, wl.fs, _cuda(wl.lo), _cuda(wl.hi), cfg)["best"].cpu().numpy()
     lo, hi = wl.lo.copy(), wl.hi.copy()
-    bad = list(range(1, 480, 3))
+    bad = list(range(1, NB, 3))
     for b in bad:
         lo[b, 3] = wl.truth[b, 3] + 20.0
         hi[b, 3] = wl.truth[b, 3] + 60.0
     lod, hid = _cuda(lo), _cuda(hi)
     fit = pt.pt_fit_blocks(xd, wl.fs, lod, hid, cfg)
     sms = torch.cuda.get_device_properties(0).multi_processor_count
-    assert len(bad) > sms and pt.pt_fit_blocks_plan(len(bad), wl.N, cfg)["tail_cluster"] > 1
+    assert len(bad) > sms * pt.pt_fit_blocks_plan(NB, wl.N, cfg)["ctas_per_sm"]
     att = pt.pt_refit_doubtful(xd, wl.fs, lod, hid, cfg, pt.make_retry_config(phi_tol=1.0, F_tol=1.0, f_floor=2.0, fdot_floor=2.0),
                                fit).cpu().numpy()
     searched = set(int(b) for b in np.nonzero(att)[0])
     # every block with wrong ranges is searched again, once; so are the two end blocks (their only border is bad and
     # they cannot be told apart from their neighbour) and the odd pair of good blocks whose own common border failed the
     # check in the short 120-generation first fit
-    assert set(bad) <= searched and {0, 479} <= searched and len(searched - set(bad)) <= 8
+    assert set(bad) <= searched and {0, NB - 1} <= searched and len(searched - set(bad)) <= 16
     assert np.all(att[bad] == 1) and att.max() == 1
     assert not np.any(fit["status"].cpu().numpy() & 4)
     d = fit["best"].cpu().numpy() - ref
-    good = [b for b in range(480) if b not in searched]
+    good = [b for b in range(NB) if b not in searched]
     assert np.array_equal(d[good], np.zeros_like(d[good]))
     assert np.max(np.abs(d[bad, 3])) < 2e-2 and np.max(np.abs(_wrap(d[bad, 2]))) < 5e-2

@@ -194,18 +194,22 @@ def test_tc_persistent_loop_block_index_quantised_and_status(pt):
     assert torch.equal(a["best"], b["best"]) and torch.equal(a["best_rss"], b["best_rss"])
 
 
-def test_automatic_choice_takes_the_tensor_core_kernel_for_config3(pt):
-    cfg = pt.make_config(D=6, NP=128, generations=1500, t0=-0.05)
-    plan = pt.pt_fit_blocks_plan(36000, 10000, cfg)
-    assert plan["threads"] == 640 and plan["cands_per_thread"] == 1
+def test_automatic_choice_is_the_run_kernel_and_the_hooks_force_the_others(pt):
+    """Automatic choice: pt_run_kernel everywhere -- 1024 threads per SM as 1, 2 or 4 CTAs, one candidate per
+    thread; PT_KERNEL=tc / classic force the other two evaluation kernels."""
+    cfg6 = pt.make_config(D=6, NP=128, generations=1500, t0=-0.05)
     cfg5 = pt.make_config(D=5, NP=128, generations=1000, t0=-0.5)
-    assert pt.pt_fit_blocks_plan(3600, 16000, cfg5)["threads"] == 512          # long D = 5 blocks stay on the FP32-pipe kernel
-    assert pt.pt_fit_blocks_plan(1024, 4096, cfg5)["threads"] == 640           # short blocks: two per CTA on the tensor-core kernel
-    assert pt.pt_fit_blocks_plan(1024, 4096, pt.make_config(D=5, NP=64, generations=10, t0=-0.5))["threads"] != 640
+    for B, N, cfg in ((36000, 10000, cfg6), (3600, 16000, cfg5), (1024, 4096, cfg5), (1024, 262144, cfg5)):
+        plan = pt.pt_fit_blocks_plan(B, N, cfg)
+        assert plan["threads"] * plan["ctas_per_sm"] == 1024 and plan["cands_per_thread"] == 1, plan
+    with _kernel("tc"):
+        assert pt.pt_fit_blocks_plan(36000, 10000, cfg6)["threads"] == 640
+    with _kernel("classic"):
+        assert pt.pt_fit_blocks_plan(3600, 16000, cfg5)["threads"] == 512
 
 
 def test_classic_kernel_still_covers_d6(pt):
-    """The automatic choice sends D = 6 to the tensor-core kernel; the FP32-pipe kernel's D = 6 path stays covered: both kernels on
+    """The automatic choice is pt_run_kernel; the D = 6 paths of the other two kernels stay covered: both on
     the same config-3 blocks against the oracle's objective, and against each other at the parity bars."""
     wl = W.config3(blocks=[100, 20000])
     a = _fit(pt, wl, "classic", seed=4)
