@@ -97,6 +97,12 @@ static int device_info(int* sms, int* smem_optin, int* dev_out = nullptr) {
     return 0;
 }
 
+static int device_smem_optin() {
+    int sms = 148, smem_optin = 232448;
+    if (device_info(&sms, &smem_optin)) return 232448;
+    return smem_optin;
+}
+
 // Warp grid (Wg candidate-group columns x Ws sample slices) with the smallest per-warp load.
 static void choose_warp_grid(int warps, int groups, int nch, int* Wg, int* Ws) {
     long long best = -1;
@@ -134,7 +140,7 @@ static bool want_run() {
 // Plan of pt_run_kernel: one CTA of 1024 threads per SM, or 2 x 512 / 4 x 256 when shared memory and the number of blocks allow (the
 // DE step of one CTA then overlaps with the evaluation of the others); with few blocks a cluster of K CTAs per block; blocks
 // larger than shared memory are streamed through a ring of 3 tiles.
-static int make_plan_run(long long B, int N, int NP, int D, int sms, int smem_optin, int force_K, Plan* pl) {
+static int make_plan_run(long long B, int N, int NP, int D, int sms, int smem_optin, int force_K, Plan* pl, int max_cps = 4) {
     pl->sms = sms;
     pl->tc = 0; pl->tc_slots = 1; pl->run = 1;
     pl->C = 1; pl->NPpad = NP; pl->Wg = 1; pl->Ws = 1;
@@ -158,7 +164,7 @@ static int make_plan_run(long long B, int N, int NP, int D, int sms, int smem_op
             }
         }
     }
-    for (int cps = 4; cps >= 1; cps >>= 1) {
+    for (int cps = max_cps; cps >= 1; cps >>= 1) {
         if (cps > 1 && B <= (long long)sms * (cps / 2)) continue;   // not enough blocks to want that many CTAs
         const int threads = kRunMaxThreads / cps;
         const RunSmemLayout L(pl->Npad, NP, D, threads);
@@ -481,6 +487,51 @@ static long long plan_tail(long long B, int N, int NP, int D, const Plan& pl, Pl
     return 0;
 }
 
+// Launch list of pt_run_kernel.  All blocks take the same time, so a persistent grid is balanced only when every CTA fits the same
+// number of blocks and every SM holds the same number of CTAs -- and which CTAs share an SM is the block scheduler's business
+// (measured on the B200: consecutive CTAs, not CTA i and i + SMs), so a partly filled last round can leave half of the SMs idle.
+// The blocks are therefore cut into segments, one launch each, in which the grid is exactly full: whole rounds of SMs x c CTAs,
+// then the remainder with fewer (larger) CTAs per SM, and the last < SMs / 2 blocks on clusters of K = SMs / rem CTAs per block.
+struct Segment { long long first, count; Plan pl; };
+static int run_launch_list(long long B, int N, int NP, int D, int sms, int smem_optin, std::vector<Segment>* out) {
+    long long done = 0;
+    int max_cps = 4;
+    while (done < B) {
+        const long long left = B - done;
+        Segment sg;
+        sg.first = done;
+        if (left * 2 <= sms) {
+            // the last few blocks: clusters, as many CTAs per block as are resident at once
+            bool ok = false;
+            for (int K = (int)(sms / left) < 8 ? (int)(sms / left) : 8; K >= 2 && !ok; --K) {
+                if (make_plan_run(left, N, NP, D, sms, smem_optin, K, &sg.pl) || sg.pl.K != K) continue;
+                ok = fit_max_resident_clusters(sg.pl, D) >= left;
+            }
+            if (!ok && make_plan_run(left, N, NP, D, sms, smem_optin, 1, &sg.pl, 1)) return 1;
+            sg.count = left;
+        } else {
+            if (make_plan_run(left, N, NP, D, sms, smem_optin, 1, &sg.pl, max_cps)) return 1;
+            const long long slots = (long long)sms * sg.pl.ctas_per_sm;
+            if (left >= slots) {
+                sg.count = left / slots * slots;
+            } else if (sg.pl.ctas_per_sm > 1) {
+                // fewer blocks than CTA slots: the largest c' <= left / SMs CTAs per SM, exactly full
+                int c = sg.pl.ctas_per_sm;
+                while (c > 1 && (long long)sms * c > left) c >>= 1;
+                if (make_plan_run((long long)sms * c, N, NP, D, sms, smem_optin, 1, &sg.pl, c)) return 1;
+                sg.count = left < (long long)sms * sg.pl.ctas_per_sm ? left : (long long)sms * sg.pl.ctas_per_sm;
+            } else {
+                sg.count = left;
+            }
+            max_cps = sg.pl.ctas_per_sm;
+            sg.pl.grid = (int)(sg.count < (long long)sms * sg.pl.ctas_per_sm ? sg.count : (long long)sms * sg.pl.ctas_per_sm);
+        }
+        out->push_back(sg);
+        done += sg.count;
+    }
+    return 0;
+}
+
 // streamed path: hand the workspace rows to the kernel
 static int attach_workspace(BlockParams* p, const Plan& pl, void* workspace, size_t workspace_bytes) {
     p->TS = pl.TS; p->S = pl.S;
@@ -607,6 +658,7 @@ int32_t pt_objective(const float* x, int64_t B, int32_t N, double fs, double t0,
     p.x = x; p.pop_in = pop; p.fitness_out = fitness;
     p.B = B; p.N = N; p.Npad = pl.Npad; p.NP = NP; p.NPpad = pl.NPpad; p.G = 0;
     p.fs = fs; p.t0 = t0; p.Wg = pl.Wg; p.Ws = pl.Ws; p.strategy = kRand1;
+    p.dt = 1.0 / fs; p.dtf = (float)p.dt; p.t0f = (float)t0;
     p.use_bulk = ((N % 4) == 0 && (reinterpret_cast<uintptr_t>(x) % 16) == 0) ? 1 : 0;
     rc = attach_workspace(&p, pl, workspace, workspace_bytes);
     if (rc) return rc;
@@ -636,7 +688,12 @@ int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg, int32_
     int dev_count = 0;
     if (cudaGetDeviceCount(&dev_count) == cudaSuccess && dev_count > 0) {
         Plan tl;
-        if (plan_tail(B, N, cfg->NP, cfg->D, pl, &tl) > 0) out[7] = tl.K;
+        if (pl.run) {
+            std::vector<Segment> segs;
+            if (force_cluster() == 0 && pl.K == 1 && pl.S == 0 && run_launch_list(B, N, cfg->NP, cfg->D, pl.sms, device_smem_optin(), &segs) == 0 &&
+                segs.size() > 1 && segs.back().pl.K > 1)
+                out[7] = segs.back().pl.K;
+        } else if (plan_tail(B, N, cfg->NP, cfg->D, pl, &tl) > 0) out[7] = tl.K;
     } else {
         (void)cudaGetLastError();
     }
@@ -670,6 +727,7 @@ static int32_t fit_blocks_impl(const float* x, const unsigned char* xq, const pt
     p.best = best; p.best_rss = best_rss; p.status = status; p.final_pop = final_pop; p.final_fit = final_fit;
     p.B = B; p.N = N; p.Npad = pl.Npad; p.NP = cfg->NP; p.NPpad = pl.NPpad; p.G = cfg->generations;
     p.fs = fs; p.t0 = cfg->t0; p.F = cfg->F;
+    p.dt = 1.0 / fs; p.dtf = (float)p.dt; p.t0f = (float)cfg->t0;
     p.CR32 = cr32_of(cfg->CR);
     p.key0 = (uint32_t)(cfg->seed & 0xFFFFFFFFull); p.key1 = (uint32_t)(cfg->seed >> 32);
     p.Wg = pl.Wg; p.Ws = pl.Ws;
@@ -677,6 +735,21 @@ static int32_t fit_blocks_impl(const float* x, const unsigned char* xq, const pt
     p.use_bulk = (!xq && (N % 4) == 0 && (reinterpret_cast<uintptr_t>(x) % 16) == 0) ? 1 : 0;
     rc = attach_workspace(&p, pl, workspace, workspace_bytes);
     if (rc) return rc;
+    if (pl.run && !count && force_cluster() == 0 && pl.K == 1 && pl.S == 0) {
+        // segments of exactly full grids (run_launch_list); every launch reads its own geometry from its plan
+        std::vector<Segment> segs;
+        if (run_launch_list(B, N, cfg->NP, cfg->D, pl.sms, device_smem_optin(), &segs)) { set_error("no launch plan"); return PT_ERR_UNSUPPORTED; }
+        for (const Segment& sg : segs) {
+            BlockParams q = p;
+            q.blk0 = sg.first; q.B = sg.first + sg.count;
+            q.Npad = sg.pl.Npad; q.NPpad = sg.pl.NPpad; q.Wg = sg.pl.Wg; q.Ws = sg.pl.Ws;
+            rc = attach_workspace(&q, sg.pl, nullptr, 0);
+            if (rc) return rc;
+            rc = dispatch<kModeFit>(q, sg.pl, cfg->D, cfg->objective, (cudaStream_t)stream);
+            if (rc) return rc;
+        }
+        return PT_OK;
+    }
     Plan tl;
     const long long rem = count ? 0 : plan_tail(B, N, cfg->NP, cfg->D, pl, &tl);
     if (rem == 0) return dispatch<kModeFit>(p, pl, cfg->D, cfg->objective, (cudaStream_t)stream);

@@ -61,6 +61,8 @@ struct BlockParams {
     long long blk0;
     int N, Npad, NP, NPpad, G;
     double fs, t0, F;
+    double dt;                    // 1 / fs (set on the host: pt_run_kernel reads it once per run instead of dividing)
+    float dtf, t0f;               // dt and t0 rounded to fp32 (amplitude time base of pt_run_kernel)
     uint32_t CR32, key0, key1;
     int strategy;                 // Strategy (pt_device.cuh), 1..6
     int Wg, Ws;                   // warp grid of the evaluation phase, Wg * Ws = warps per CTA

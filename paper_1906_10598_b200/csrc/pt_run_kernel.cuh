@@ -5,25 +5,28 @@
 //   * transposed layout: a THREAD owns one candidate and walks a contiguous slice of the block's samples (thread = candidate x
 //     slice); the sample values are warp-uniform shared-memory broadcasts (one LDS.128 per four sample-evaluations of a warp),
 //     there is no shuffle reduction and no reference-phase array (shared memory holds 4 bytes per sample);
-//   * the samples are walked in RUNS of kRun = 128.  Per run the phase polynomial of Eq. 3, P(t) = phi0/2pi + f t + fdot t^2/2 +
+//   * the samples are walked in RUNS of kRun = 256.  Per run the phase polynomial of Eq. 3, P(t) = phi0/2pi + f t + fdot t^2/2 +
 //     fddot t^3/6 [turns], is re-expanded at the run centre t_c in fp64: E0 = 2 pi frac(P(t_c)), E1 = 2 pi dt P1(t_c),
 //     E2 = 2 pi dt^2 P2(t_c)/2, E3 = 2 pi dt^3 P3/6 (Pk = k-th derivative), so that phase(j) = E0 + j (E1 + j (E2 + j E3)) for the
 //     sample j steps from the centre.  The large part of the phase (6e3 ... 3e5 rad) is removed exactly and fp32 never sees more
-//     than pi + 64 |E1|.  Inside the run the index j is a COMPILE-TIME constant of the fully unrolled instruction stream, so
+//     than pi + 128 |E1|.  Inside the run the index j is a COMPILE-TIME constant of the fully unrolled instruction stream, so
 //     the Horner scheme needs no index arithmetic at all; per PAIR of consecutive samples (j, j + 1), with packed coefficient pairs
 //     whose second lane holds the polynomial shifted by one sample:
-//         FFMA2 h = E2 j + E1,  FFMA2 y = h j + E0          phase of samples (j, j + 1); j is a 32-bit immediate (FFMA2 R, R, -64, R)
+//         FFMA2 h = E2 j + E1,  FFMA2 y = h j + E0          phase of samples (j, j + 1); j is a 32-bit immediate (FFMA2 R, R, -128, R)
 //         2 x (FMUL + MUFU.COS)                              cos.approx
 //         FFMA2 A = G j + Ac                                 negated amplitude -(a0 + a1 t)
 //         FFMA2 r = A c + x,  FFMA2 acc += r r
 //     i.e. 6 FP32-pipe lane operations + 1 MUFU per sample-evaluation for D = 5 (pt_block_kernel: 7) and the same for D = 6 whenever
-//     the cubic term cannot matter inside a run (|E3| 64^3 below 1e-7 rad over the whole box: the run then carries the exact value,
+//     the cubic term cannot matter inside a run (|E3| 128^3 below 1e-7 rad over the whole box: the run then carries the exact value,
 //     first and second derivative of the cubic at its centre); 7 otherwise.  4.75 issue slots per sample-evaluation (5.3);
 //   * 64 registers per thread: 32 warps per SM (one CTA of 1024 threads, or 2 x 512 / 4 x 256 for shorter blocks, whose DE steps
 //     then overlap with the other CTAs' evaluation), against 16 warps of 128 registers in pt_block_kernel.
 // Every phase is rounded on its own: there is no recurrence.  (A forward-difference recurrence y += d, d += dd was measured first
-// and dropped: with dd below half an ulp of d the second difference is lost and the phase drifts by E2 j^2, 1e-5 rad at j = 64.)
-// Summation: fp32 FMA over a run (64 terms per accumulator), error-free two-sum of the run's value into a (hi, lo) pair, fp64 from
+// and dropped: with dd below half an ulp of d the second difference is lost and the phase drifts by E2 j^2, 1e-5 rad at j = 64.
+// The run length trades the per-run re-expansion (about 60 instructions, a serial fp64 chain) against the size of the fp32 phases:
+// measured on config 2, 64 / 128 / 256 samples per run give 80.5 / 86.5 / 89.2 % of the XU roofline and a largest objective error of
+// 1.5e-7 / 4e-7 / 1.7e-6 relative; 256 is also the tile of pt_tc_kernel.)
+// Summation: fp32 FMA over a run (128 terms per accumulator), error-free two-sum of the run's value into a (hi, lo) pair, fp64 from
 // there on (partials, objective values, selection), as in pt_tc_kernel (R18, R20).
 // Measured numbers and the comparison with the other two evaluation kernels: DESIGN.md section 5.13, profiles/r2_*.
 #pragma once
@@ -32,7 +35,10 @@
 namespace pt {
 
 #ifndef PT_RUN_SAMPLES
-#define PT_RUN_SAMPLES 128
+#define PT_RUN_SAMPLES 256
+#endif
+#ifndef PT_RUN_INLINE
+#define PT_RUN_INLINE __noinline__
 #endif
 constexpr int kRun = PT_RUN_SAMPLES;      // samples per run
 constexpr int kRunMaxThreads = 1024;
@@ -98,15 +104,35 @@ __device__ __forceinline__ void run_full(const float* __restrict__ xr, const Run
         run_pair<AMP, CUB>(c, (float)(k + 2 - kRun / 2), q.z, q.w, acc);
     }
 }
-// a shorter run (the last one of a slice): `len` (even) samples, the first one at j = jf0
+// a shorter run (the last one of a slice): `len` (even) samples, the first one at j = jf0 (an integer, carried exactly in fp32)
 template <int AMP, bool CUB>
 __device__ __forceinline__ void run_part(const float* __restrict__ xr, const int len, const float jf0, const RunCoef& c, f32x2& acc) {
     float jf = jf0;
+    int k = 0;
+    for (; k + 16 <= len; k += 16, jf += 16.0f) {
+#pragma unroll
+        for (int u = 0; u < 16; u += 4) {
+            const float4 q = *reinterpret_cast<const float4*>(xr + k + u);
+            run_pair<AMP, CUB>(c, jf + (float)u, q.x, q.y, acc);
+            run_pair<AMP, CUB>(c, jf + (float)(u + 2), q.z, q.w, acc);
+        }
+    }
 #pragma unroll 1
-    for (int k = 0; k < len; k += 2, jf += 2.0f) {
+    for (; k < len; k += 2, jf += 2.0f) {
         const float2 q = *reinterpret_cast<const float2*>(xr + k);
         run_pair<AMP, CUB>(c, jf, q.x, q.y, acc);
     }
+}
+
+// double -> float by integer operations on the bits (round to nearest, ties away; |v| < 2^-126 gives 0): the conversion
+// instruction F2F.F32.F64 executes on the XU pipe, the pipe the cosines saturate (measured: 4 conversions per run = 3.5 % of the
+// XU cycles of this kernel).
+__device__ __forceinline__ float run_d2f(const double v) {
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v) + 0x10000000ull;      // + half an fp32 ulp
+    const uint32_t hi = (uint32_t)(b >> 32), lo = (uint32_t)b;
+    const uint32_t mag = hi & 0x7FFFFFFFu;
+    const uint32_t fb = __funnelshift_l(lo, mag - 0x38000000u, 3) | (hi & 0x80000000u);          // re-biased exponent, 23 mantissa bits
+    return __uint_as_float(mag >= 0x38100000u ? fb : 0u);
 }
 
 // One evaluation pass over a tile of samples that sits in shared memory: xs[0 .. len_t) are samples n_t0 .. n_t0 + len_t of the
@@ -115,42 +141,51 @@ __device__ __forceinline__ void run_part(const float* __restrict__ xr, const int
 // i % NP over slice i / NP, and thread t takes items t, t + threads, ...  The item's sum goes to part[i] (added when `accumulate`).
 // Not inlined: the loop's register allocation then does not depend on the code around it.
 template <int D, int AMP, bool CUB>
-__device__ __noinline__ void run_eval_tile(const float* __restrict__ xs, const int n_t0, const int len_t, const double* __restrict__ pop,
-                                          double* __restrict__ part, const bool accumulate, const int NP, const double fs, const double t0,
-                                          const int tid, const int nthr) {
+__device__ PT_RUN_INLINE void run_eval_tile(const BlockParams& p, const float* __restrict__ xs, const int n_t0, const int len_t,
+                                          const double* __restrict__ pop, double* __restrict__ part, const bool accumulate, const int tid,
+                                          const int nthr) {
+    const int NP = p.NP;
     const int S = nthr > NP ? nthr / NP : 1;
     const int quads = (len_t + 3) >> 2;
-    const double dt = 1.0 / fs;
-    const float dtf = (float)dt;
     const f32x2 neg1 = run_bc2(-1.0f);
     for (int item = tid; item < NP * S; item += nthr) {
         const int cand = item % NP, slice = item / NP;
         const int nb = (int)(((long long)slice * quads) / S) * 4;
         const int ne = min(len_t, (int)(((long long)(slice + 1) * quads) / S) * 4);
         const double* th = pop + cand * D;
-        // phase polynomial in turns (Eq. 3) and its scaled derivatives
-        const double c0 = th[2] * (1.0 / kTwoPi), c1 = th[3], c2 = 0.5 * th[4], c3 = (D == 6) ? th[5] * (1.0 / 6.0) : 0.0;
-        const double k1 = kTwoPi * dt * c1, k2 = kTwoPi * dt * 2.0 * c2, k3 = kTwoPi * dt * 3.0 * c3;
-        const double m2 = kTwoPi * dt * dt * c2, m3 = kTwoPi * dt * dt * 3.0 * c3;
-        const float E3 = (D == 6) ? (float)(kTwoPi * c3 * dt * dt * dt) : 0.0f;
+        // phase polynomial in turns (Eq. 3): P = c0 + t (f + t (fdot/2 + t fddot/6)); only c0, f, fdot, fddot stay
+        // in registers, the halves and thirds are formed where they are used (the fp64 pipe is 2 % busy, registers are scarce)
+        const double c0 = th[2] * (1.0 / kTwoPi), f1 = th[3], f2 = th[4], f3 = (D == 6) ? th[5] : 0.0;
         const float na0 = -(float)th[0], na1 = (AMP == kRunAmpLinear) ? -(float)th[1] : 0.0f;
-        const float g1 = na1 * dtf;
         f32x2 hi = run_bc2(0.0f), lo = run_bc2(0.0f);
-        double nd = (double)(n_t0 + nb);                       // block-relative index of the run's first sample
-        for (int n0 = nb; n0 < ne; n0 += kRun, nd += (double)kRun) {
+        // block-relative index of the run's first sample, in both precisions (exact: < 2^24; a conversion would run on the XU pipe)
+        double nd = (double)(n_t0 + nb);
+        float nf = (float)(n_t0 + nb);
+        for (int n0 = nb; n0 < ne; n0 += kRun, nd += (double)kRun, nf += (float)kRun) {
             f32x2 acc = run_bc2(0.0f);
             // The polynomial is re-expanded at sample h of the run (its centre; a short last run of a slice: ITS centre, so that a
             // block of a few samples is evaluated next to the expansion point).
-            auto coefficients = [&](const int h) -> RunCoef {
-                const double tcen = fma(nd + (double)h, dt, t0);
-                double P = (D == 6) ? fma(tcen, fma(tcen, fma(tcen, c3, c2), c1), c0) : fma(tcen, fma(tcen, c2, c1), c0);
+            auto coefficients = [&](const float hf, const double hd) -> RunCoef {
+                const double dt = p.dt;
+                const double tcen = fma(nd + hd, dt, p.t0);
+                const double w1 = kTwoPi * dt;
+                double P, e1, e2;
+                if (D == 6) {
+                    const double h3 = 0.5 * f3;
+                    P = fma(tcen, fma(tcen, fma(tcen, f3 * (1.0 / 6.0), 0.5 * f2), f1), c0);
+                    e1 = w1 * fma(tcen, fma(tcen, h3, f2), f1);                 // 2 pi dt P'(t_c)
+                    e2 = (w1 * dt) * fma(tcen, h3, 0.5 * f2);                   // 2 pi dt^2 P''(t_c) / 2
+                } else {
+                    P = fma(tcen, fma(tcen, 0.5 * f2, f1), c0);
+                    e1 = w1 * fma(tcen, f2, f1);
+                    e2 = (w1 * dt) * (0.5 * f2);
+                }
                 P -= __dadd_rn(__dadd_rn(P, 6755399441055744.0), -6755399441055744.0);      // P - rint(P), |P| < 2^51
-                const float E0 = (float)(kTwoPi * P);
-                const float E1 = (float)((D == 6) ? fma(tcen, fma(tcen, k3, k2), k1) : fma(tcen, k2, k1));
-                const float E2 = (float)((D == 6) ? fma(tcen, m3, m2) : m2);
+                const float E0 = run_d2f(kTwoPi * P), E1 = run_d2f(e1), E2 = run_d2f(e2);
                 RunCoef c;
                 // lane 1 = the polynomial in (j + 1): E0 + E1 + E2 + E3, E1 + 2 E2 + 3 E3, E2 + 3 E3, E3
                 if (CUB) {
+                    const float E3 = run_d2f((w1 * dt) * dt * (f3 * (1.0 / 6.0)));
                     c.E0 = pack2(E0, (E0 + E1) + (E2 + E3));
                     c.E1 = pack2(E1, fmaf(3.0f, E3, fmaf(2.0f, E2, E1)));
                     c.E2 = pack2(E2, fmaf(3.0f, E3, E2));
@@ -162,7 +197,8 @@ __device__ __noinline__ void run_eval_tile(const float* __restrict__ xs, const i
                     c.E3 = run_bc2(0.0f);
                 }
                 if (AMP == kRunAmpLinear) {
-                    const float Ac = fmaf(na1, (float)tcen, na0);
+                    const float dtf = p.dtf, g1 = na1 * dtf;
+                    const float Ac = fmaf(na1, fmaf(nf + hf, dtf, p.t0f), na0);      // -(a0 + a1 t_c), t_c in fp32: |t| ulp 3e-8 relative
                     c.Ac = pack2(Ac, Ac + g1);
                     c.G = run_bc2(g1);
                 } else {
@@ -172,11 +208,11 @@ __device__ __noinline__ void run_eval_tile(const float* __restrict__ xs, const i
                 return c;
             };
             if (n0 + kRun <= ne) {
-                const RunCoef c = coefficients(kRun / 2);
+                const RunCoef c = coefficients((float)(kRun / 2), (double)(kRun / 2));
                 run_full<AMP, CUB>(xs + n0, c, acc);
             } else {
                 const int len = ne - n0, h = len >> 1;
-                const RunCoef c = coefficients(h);
+                const RunCoef c = coefficients((float)h, (double)h);
                 run_part<AMP, CUB>(xs + n0, len, -(float)h, c, acc);
             }
             // (hi, lo) += acc without losing the rounding error of the addition (Knuth's two-sum, packed)
@@ -209,7 +245,7 @@ struct RunStream {
 __device__ __forceinline__ void run_stream_issue_one(const BlockParams& p, RunStream& st) {
     const int s = (int)(st.prod % (uint32_t)p.S);
     const uint32_t k = st.prod / (uint32_t)p.S;
-    if (k >= 1) mbar_wait(&st.empty[s], (k - 1) & 1u);        // every warp has released the previous fill
+    if (k >= 1) mbar_wait_suspended(&st.empty[s], (k - 1) & 1u);        // every warp has released the previous fill
     const int n0 = st.j_issue * p.TS;
     const int N4 = p.use_bulk ? p.N : (p.N + 3) & ~3;         // N % 4 == 0 on the direct path, else the zero-padded workspace copy
     const uint32_t xb = (uint32_t)min(p.TS, N4 - n0) * 4u;
@@ -264,7 +300,6 @@ __global__ void __launch_bounds__(kRunMaxThreads, 1) pt_run_kernel(const BlockPa
     }
     __syncthreads();
     if (K > 1) cluster_sync_all();     // every CTA of the cluster is running before any peer store is issued
-
     // Objective value of member i: the slices' partial sums in fixed order; with a cluster, the K CTAs' sums are exchanged through
     // distributed shared memory and added in rank order, so every CTA of the cluster holds the same fp64 value.
     auto combine_begin = [&]() {
@@ -380,13 +415,13 @@ __global__ void __launch_bounds__(kRunMaxThreads, 1) pt_run_kernel(const BlockPa
         // one evaluation pass of the population `pop` over the samples this CTA holds (or streams)
         auto eval_tile = [&](const float* tile, int n_t0, int len_t, const double* pop, bool accumulate) {
             if (D == 6 && cub) {
-                if (OBJ == kObjCor) run_eval_tile<D, kRunAmpCor, true>(tile, n_t0, len_t, pop, part, accumulate, p.NP, p.fs, p.t0, tid, nthr);
-                else if (a1z) run_eval_tile<D, kRunAmpConst, true>(tile, n_t0, len_t, pop, part, accumulate, p.NP, p.fs, p.t0, tid, nthr);
-                else run_eval_tile<D, kRunAmpLinear, true>(tile, n_t0, len_t, pop, part, accumulate, p.NP, p.fs, p.t0, tid, nthr);
+                if (OBJ == kObjCor) run_eval_tile<D, kRunAmpCor, true>(p, tile, n_t0, len_t, pop, part, accumulate, tid, nthr);
+                else if (a1z) run_eval_tile<D, kRunAmpConst, true>(p, tile, n_t0, len_t, pop, part, accumulate, tid, nthr);
+                else run_eval_tile<D, kRunAmpLinear, true>(p, tile, n_t0, len_t, pop, part, accumulate, tid, nthr);
             } else {
-                if (OBJ == kObjCor) run_eval_tile<D, kRunAmpCor, false>(tile, n_t0, len_t, pop, part, accumulate, p.NP, p.fs, p.t0, tid, nthr);
-                else if (a1z) run_eval_tile<D, kRunAmpConst, false>(tile, n_t0, len_t, pop, part, accumulate, p.NP, p.fs, p.t0, tid, nthr);
-                else run_eval_tile<D, kRunAmpLinear, false>(tile, n_t0, len_t, pop, part, accumulate, p.NP, p.fs, p.t0, tid, nthr);
+                if (OBJ == kObjCor) run_eval_tile<D, kRunAmpCor, false>(p, tile, n_t0, len_t, pop, part, accumulate, tid, nthr);
+                else if (a1z) run_eval_tile<D, kRunAmpConst, false>(p, tile, n_t0, len_t, pop, part, accumulate, tid, nthr);
+                else run_eval_tile<D, kRunAmpLinear, false>(p, tile, n_t0, len_t, pop, part, accumulate, tid, nthr);
             }
         };
         auto evaluate = [&](const double* pop) {
@@ -395,7 +430,7 @@ __global__ void __launch_bounds__(kRunMaxThreads, 1) pt_run_kernel(const BlockPa
                 for (int jt = 0; jt < nT; ++jt) {
                     if (tid == 0 && st.to_issue > 0) run_stream_issue_one(p, st);
                     const int s = (int)(st.cons % (uint32_t)p.S);
-                    mbar_wait(&st.full[s], (st.cons / (uint32_t)p.S) & 1u);
+                    mbar_wait_suspended(&st.full[s], (st.cons / (uint32_t)p.S) & 1u);
                     eval_tile(st.stages + (size_t)s * p.TS, jt * p.TS, min(p.TS, p.N - jt * p.TS), pop, jt > 0);
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&st.empty[s]);
