@@ -37,7 +37,17 @@ SM_MAX_MHZ = 1965.0
 XU_PEAK = SM_COUNT * XU_LANES_PER_SM * SM_MAX_MHZ * 1e6     # 4.65e12 sample-evaluations/s, DESIGN.md "Roofline"
 # dram__bytes_read.sum + dram__bytes_write.sum of the DE-kernel launches of one step, from an `ncu --set full` capture of the
 # same command (profile file named beside the number); reported as roofline.traffic_ncu, never as a live measurement
-NCU_TRAFFIC = {"config2": {"bytes": 2.44e8, "source": "profiles/r1e_bench_launches.md (main + tail launch of one step)"}}
+NCU_TRAFFIC = {"config2": {"bytes": 2.31e8, "source": "profiles/r2_bench_launches.md (the two DE-kernel launches of one step)"}}
+
+
+def kernel_name(plan: dict, wl) -> str:
+    """Which evaluation kernel the plan runs (include/pt.h, pt_fit_blocks_launches): told from its geometry."""
+    obj = "cor" if wl.de["objective"] else "chi2"
+    if plan["threads"] == 640:
+        return "pt_tc_kernel<D=%d,fit,%s> (phase by tcgen05.mma kind::tf32)" % (wl.de["D"], obj)
+    if plan["cands_per_thread"] == 1:
+        return "pt_run_kernel<D=%d,fit,%s,%s> (thread = candidate, run-local Horner)" % (wl.de["D"], "resident" if plan["resident"] else "streamed", obj)
+    return "pt_block_kernel<C=%d,D=%d,fit,%s>" % (plan["cands_per_thread"], wl.de["D"], obj)
 
 
 def peak_probe(kind: int) -> float:
@@ -263,7 +273,7 @@ def run_sweep(args, dev):
     Ns = [int(v) for v in args.sweep_n.split(",")]
     NPs = [int(v) for v in args.sweep_np.split(",")]
     B, G = args.sweep_blocks, args.sweep_generations
-    points, tot_units, tot_ms = [], 0.0, 0.0
+    points, tot_units, tot_ms, n_launches = [], 0.0, 0.0, 0
     sampler = ClockSampler(dev.index or 0)
     sampler.start()
     for N in Ns:
@@ -272,6 +282,7 @@ def run_sweep(args, dev):
         for NP in NPs:
             cfg = pt.make_config(D=5, NP=NP, generations=G, F=0.5, CR=0.9, seed=1, t0=wl.t0)
             plan = pt.pt_fit_blocks_plan(B, N, cfg)
+            launches = pt.pt_fit_blocks_launches(B, N, cfg)
             for _ in range(max(1, args.warmup if N * NP < 2 ** 22 else 1)):
                 pt.pt_fit_blocks(x, wl.fs, lo, hi, cfg)
             torch.cuda.synchronize()
@@ -283,6 +294,7 @@ def run_sweep(args, dev):
             e1.record()
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1) / steps
+            n_launches += steps * len(launches)
             units = float(B) * NP * (G + 1) * N
             rate = units / (ms * 1e-3)
             tot_units += units
@@ -290,7 +302,7 @@ def run_sweep(args, dev):
             ok = float((r["best_rss"] > 0).float().mean().item())
             points.append({"N": N, "NP": NP, "ms": ms, "sample_evals_per_s": rate, "fitness_evals_per_s": rate / N,
                            "xu_frac": rate / XU_PEAK, "resident": plan["resident"], "threads": plan["threads"],
-                           "ctas_per_sm": plan["ctas_per_sm"], "smem": plan["smem"], "finite": ok})
+                           "ctas_per_sm": plan["ctas_per_sm"], "smem": plan["smem"], "launches": len(launches), "finite": ok})
         del x
     clocks = sampler.stop()
     line = {"metric": METRIC, "value": tot_units / (tot_ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
@@ -301,7 +313,7 @@ def run_sweep(args, dev):
             "roofline": {"bound": "alu", "peak": XU_PEAK / 1e12, "unit": "T sample-evals/s (1 MUFU cosine each)",
                          "achieved": tot_units / (tot_ms * 1e-3) / 1e12, "frac": tot_units / (tot_ms * 1e-3) / XU_PEAK,
                          "traffic": None},
-            "points": points, "clocks": clocks, "gpu_launches": len(points)}
+            "points": points, "clocks": clocks, "gpu_launches": n_launches}
     print(json.dumps(line), flush=True)
 
 
@@ -383,7 +395,8 @@ def run_strong(args, rank: int, local_rank: int, world: int, dev):
                 "e2e": {"value": units / e2e_s, "unit": UNIT, "ms_per_step": 1e3 * e2e_s,
                         "h2d_bytes_per_step": int(sum(t.numel() * t.element_size() for t in (x_h, lo_h, hi_h))),
                         "d2h_bytes_per_step": int(sum(t.numel() * t.element_size() for t in out))},
-                "gpu_launches": args.steps * (2 + 2 + len([m for m in m_int if B // m > 0]))}
+                # this rank's DE-kernel launches + 2 Doppler kernels + one kernel per integration interval, per step
+                "gpu_launches": args.steps * (len(pt.pt_fit_blocks_launches(wl.B, wl.N, cfg)) + 2 + len([m for m in m_int if B // m > 0]))}
         print(json.dumps(line), flush=True)
     dist.destroy_process_group()
 
@@ -461,6 +474,8 @@ def main():
     cfg = pt.make_config(D=wl.de["D"], NP=wl.de["NP"], generations=wl.de["generations"], F=wl.de["F"], CR=wl.de["CR"],
                          seed=1 + rank, t0=wl.t0, strategy=wl.de["strategy"], objective=wl.de["objective"])
     plan = pt.pt_fit_blocks_plan(wl.B, wl.N, cfg)
+    launches = pt.pt_fit_blocks_launches(wl.B, wl.N, cfg)
+    plan["launches"] = launches
     m_int = [max(1, int(round(tc / wl.T))) for tc in (1.0, 10.0, 60.0)]
     quant, qkw = None, {}
     if args.quant:      # the receiver's recording format (Table 3): packed samples, unpacked in-kernel while staging
@@ -552,9 +567,7 @@ def main():
                 # (a committed profile, not this run) ride along as traffic_ncu
                 "traffic": algorithmic_traffic(wl, args.quant),
                 "traffic_ncu": NCU_TRAFFIC.get(args.workload) if not (wl.de["objective"] or args.quant or args.strategy) else None,
-                "kernel": ("pt_tc_kernel<D=%d,fit,%s> (phase by tcgen05.mma kind::tf32)" % (wl.de["D"], "cor" if wl.de["objective"] else "chi2"))
-                if plan["threads"] == 640 else
-                "pt_block_kernel<C=%d,D=%d,fit,%s>" % (plan["cands_per_thread"], wl.de["D"], "cor" if wl.de["objective"] else "chi2"),
+                "kernel": kernel_name(plan, wl),
                 "kernel_ms": fit_ms, "peak_source": "derived: 148 SMs x 16 MUFU lanes x 1965 MHz (DESIGN.md); "
                 "MEASURED_PEAKS.json holds no ALU peak",
                 "frac_at_sampled_clock": achieved / (SM_COUNT * XU_LANES_PER_SM * sm_mhz * 1e6),
@@ -604,9 +617,9 @@ def main():
             "real_time_factor": wl.B * wl.T * world / (ms_per_step * 1e-3),
             "fitness_evals_per_s": value / wl.N, "fit_ms": fit_ms, "doppler_products_ms": prod_ms, "plan": plan,
             "roofline": roofline, "clocks": clocks,
-            # per step: pt_block_kernel (+ a second, cluster launch for the last partial wave), 2 Doppler kernels (per-block
-            # columns, prefix scan) and one kernel per integration interval
-            "gpu_launches": args.steps * ((2 if plan.get("tail_cluster") else 1) + 2 + len([m for m in m_int if wl.B // m > 0])),
+            # per step: the DE-kernel launches (pt_fit_blocks_launches: segments of exactly full grids), 2 Doppler kernels
+            # (per-block columns, prefix scan) and one kernel per integration interval
+            "gpu_launches": args.steps * (len(launches) + 2 + len([m for m in m_int if wl.B // m > 0])),
             "peaks_file": _peaks().get("when")}
     if quant is not None:
         line["config"]["samples"] = "%d-bit packed (Table 3), unpacked in-kernel" % args.quant

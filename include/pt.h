@@ -331,6 +331,17 @@ PT_API int32_t pt_init_population(const double* lo, const double* hi, const uint
  * The environment variable PT_CLUSTER = 1..8 overrides the automatic cluster size and disables the tail launch (tests and tuning). */
 PT_API int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg /*[host]*/, int32_t out[8] /*[host]*/);
 
+/* The DE-kernel launches pt_fit_blocks issues for B blocks (for reporting; needs a device).  Blocks all take the same time, so the
+ * library cuts them into segments whose grids are exactly full: whole rounds of SMs x c CTAs, the remainder with fewer, larger CTAs
+ * per SM, the last few blocks on clusters.  Launch k is described by out[5 k .. 5 k + 4] = first block, number of blocks, grid,
+ * threads per CTA, CTAs per data block (cluster size).  Returns the number of launches (at most `max_launches` are written), or a
+ * negative pt_status.
+ * Evaluation kernels (row a5: Eq. 2-4): pt_run_kernel (thread = candidate, run-local Horner; the automatic choice),
+ * pt_block_kernel (lanes own samples, reference-phase array), pt_tc_kernel (phase on the tensor cores; NP <= 128).  The environment
+ * variable PT_KERNEL = run | classic | tc forces one of them where it applies (tests and A/B measurements); results agree within
+ * the tolerances of the objective (fp32 rounding differs), random streams and trial vectors are identical. */
+PT_API int32_t pt_fit_blocks_launches(int64_t B, int32_t N, const pt_de_config* cfg /*[host]*/, int32_t* out /*[host]*/, int32_t max_launches);
+
 PT_API const char* pt_last_error_string(void);
 PT_API const char* pt_version(void);
 

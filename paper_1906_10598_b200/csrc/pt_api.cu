@@ -140,6 +140,25 @@ static bool want_run() {
 // Plan of pt_run_kernel: one CTA of 1024 threads per SM, or 2 x 512 / 4 x 256 when shared memory and the number of blocks allow (the
 // DE step of one CTA then overlaps with the evaluation of the others); with few blocks a cluster of K CTAs per block; blocks
 // larger than shared memory are streamed through a ring of 3 tiles.
+// Sample slices of pt_run_kernel's evaluation: NP x S work items over `threads` threads, `len` samples per tile.  Picks the S that
+// maximises (thread utilisation in whole rounds) x (useful share of a run: a run of L samples pays about 32 sample-evaluations of
+// re-expansion), smallest S on ties; at most two rounds of items.
+static int choose_slices(int NP, int threads, int len) {
+    int best = 1;
+    double best_score = -1.0;
+    const int cap = 2 * (threads > NP ? threads : NP);
+    for (int S = 1; S <= 64 && (long long)NP * S <= cap; ++S) {
+        const int per = len / S;
+        if (S > 1 && per < 64) break;
+        const long long items = (long long)NP * S, rounds = (items + threads - 1) / threads;
+        const double util = (double)items / (double)(rounds * threads);
+        const double L = per < kRun ? (double)per : (double)kRun;
+        const double score = util * L / (L + 32.0);
+        if (score > best_score + 1e-9) { best_score = score; best = S; }
+    }
+    return best;
+}
+
 static int make_plan_run(long long B, int N, int NP, int D, int sms, int smem_optin, int force_K, Plan* pl, int max_cps = 4) {
     pl->sms = sms;
     pl->tc = 0; pl->tc_slots = 1; pl->run = 1;
@@ -154,10 +173,13 @@ static int make_plan_run(long long B, int N, int NP, int D, int sms, int smem_op
         while (K * 2 <= 8 && (long long)B * (K * 2) <= sms && N / (K * 2) >= 2 * kRun) K *= 2;
         if (force_K > 0) { K = force_K; while (K > 1 && quads / K < 1) --K; }
         if (K > 1) {
+            // (splitting the cluster further into 2 x 512 or 4 x 256-thread CTAs per SM, so that the replicated DE step of one block
+            // overlaps with the evaluation of another, was measured on config 1 and lost: 26.8 / 27.7 ms against 21.3 ms)
             const int NresMax = ((quads + K - 1) / K + 1) * 4;
-            const RunSmemLayout L(NresMax, NP, D, kRunMaxThreads, 0, 0, K);
+            const int slices = choose_slices(NP, kRunMaxThreads, N / K);
+            const RunSmemLayout L(NresMax, NP, D, slices, 0, 0, K);
             if (L.total <= smem_optin) {
-                pl->threads = kRunMaxThreads; pl->ctas_per_sm = 1; pl->smem = L.total; pl->K = K; pl->NpadS = NresMax;
+                pl->threads = kRunMaxThreads; pl->ctas_per_sm = 1; pl->smem = L.total; pl->K = K; pl->NpadS = NresMax; pl->Ws = slices;
                 const long long want = (long long)(sms / K) * K;
                 pl->grid = (int)((long long)B * K < want ? (long long)B * K : want);
                 return 0;
@@ -167,10 +189,11 @@ static int make_plan_run(long long B, int N, int NP, int D, int sms, int smem_op
     for (int cps = max_cps; cps >= 1; cps >>= 1) {
         if (cps > 1 && B <= (long long)sms * (cps / 2)) continue;   // not enough blocks to want that many CTAs
         const int threads = kRunMaxThreads / cps;
-        const RunSmemLayout L(pl->Npad, NP, D, threads);
+        const int slices = choose_slices(NP, threads, N);
+        const RunSmemLayout L(pl->Npad, NP, D, slices);
         if (L.total > smem_optin) continue;
         if ((long long)(L.total + 1024) * cps > per_sm_total) continue;
-        pl->threads = threads; pl->ctas_per_sm = cps; pl->smem = L.total;
+        pl->threads = threads; pl->ctas_per_sm = cps; pl->smem = L.total; pl->Ws = slices;
         const long long want = (long long)sms * cps;
         pl->grid = (int)(B < want ? B : want);
         return 0;
@@ -178,9 +201,10 @@ static int make_plan_run(long long B, int N, int NP, int D, int sms, int smem_op
     // streamed
     pl->resident = 0;
     for (int TS = 16384; TS >= 1024; TS >>= 1) {
-        const RunSmemLayout L(pl->Npad, NP, D, kRunMaxThreads, TS, 3);
+        const int slices = choose_slices(NP, kRunMaxThreads, TS);
+        const RunSmemLayout L(pl->Npad, NP, D, slices, TS, 3);
         if (L.total > smem_optin) continue;
-        pl->threads = kRunMaxThreads; pl->ctas_per_sm = 1; pl->smem = L.total; pl->TS = TS; pl->S = 3;
+        pl->threads = kRunMaxThreads; pl->ctas_per_sm = 1; pl->smem = L.total; pl->TS = TS; pl->S = 3; pl->Ws = slices;
         pl->grid = (int)(B < sms ? B : sms);
         pl->ws_bytes = (size_t)pl->grid * pl->Npad * sizeof(float);      // aligned fp32 copies of unaligned / quantised rows
         return 0;
@@ -514,6 +538,10 @@ static int run_launch_list(long long B, int N, int NP, int D, int sms, int smem_
             const long long slots = (long long)sms * sg.pl.ctas_per_sm;
             if (left >= slots) {
                 sg.count = left / slots * slots;
+            } else if (sg.pl.ctas_per_sm > 1 && (long long)NP * N <= 65536) {
+                // blocks so short that a generation is bound by the latency of its DE step, not by the XU pipe (NP N / 14.4 cycles of
+                // evaluation against ~4500): larger CTAs would not run them faster, so the remainder stays one partly filled round
+                sg.count = left;
             } else if (sg.pl.ctas_per_sm > 1) {
                 // fewer blocks than CTA slots: the largest c' <= left / SMs CTAs per SM, exactly full
                 int c = sg.pl.ctas_per_sm;
@@ -698,6 +726,29 @@ int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg, int32_
         (void)cudaGetLastError();
     }
     return PT_OK;
+}
+
+int32_t pt_fit_blocks_launches(int64_t B, int32_t N, const pt_de_config* cfg, int32_t* out, int32_t max_launches) {
+    if (!cfg || (!out && max_launches > 0)) { set_error("null pointer argument"); return PT_ERR_INVALID_ARG; }
+    int rc = check_common(B, N, 1.0, cfg->NP, cfg->D);
+    if (rc) return rc;
+    Plan pl;
+    rc = plan_for(B, N, cfg->NP, cfg->D, &pl, true, 0, cfg->objective);
+    if (rc) return rc;
+    std::vector<Segment> segs;
+    if (pl.run && force_cluster() == 0 && pl.K == 1 && pl.S == 0) {
+        if (run_launch_list(B, N, cfg->NP, cfg->D, pl.sms, device_smem_optin(), &segs)) { set_error("no launch plan"); return PT_ERR_UNSUPPORTED; }
+    } else {
+        Plan tl;
+        const long long rem = plan_tail(B, N, cfg->NP, cfg->D, pl, &tl);
+        segs.push_back(Segment{0, B - rem, pl});
+        if (rem > 0) segs.push_back(Segment{B - rem, rem, tl});
+    }
+    for (size_t k = 0; k < segs.size() && (int32_t)k < max_launches; ++k) {
+        out[5 * k + 0] = (int32_t)segs[k].first; out[5 * k + 1] = (int32_t)segs[k].count; out[5 * k + 2] = segs[k].pl.grid;
+        out[5 * k + 3] = segs[k].pl.threads; out[5 * k + 4] = segs[k].pl.K;
+    }
+    return (int32_t)segs.size();
 }
 
 static int32_t fit_blocks_impl(const float* x, const unsigned char* xq, const pt_quant* quant, int64_t row_bytes, int64_t B,

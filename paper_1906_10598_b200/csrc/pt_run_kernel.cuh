@@ -49,7 +49,8 @@ struct RunSmemLayout {
     int off_bar, off_xs, off_popA, off_popT, off_box, off_fit, off_part, off_xpart, total;
     __host__ __device__ static int align_up(int v, int a) { return (v + a - 1) / a * a; }
     // Nres: samples this CTA keeps resident (its slice when K > 1); TS/S: tile samples and ring stages of the streamed path
-    __host__ __device__ RunSmemLayout(int Nres, int NP, int D, int threads, int TS = 0, int S = 0, int K = 1) {
+    // slices: sample slices of the evaluation (work items = NP x slices)
+    __host__ __device__ RunSmemLayout(int Nres, int NP, int D, int slices, int TS = 0, int S = 0, int K = 1) {
         int o = 0;
         off_bar = o; o += kBarBytes;               // [0] staging barrier, [1..S] full, [1+S..2S] empty
         off_xs = o; o += (S > 0) ? S * TS * 4 : align_up(Nres, 4) * 4;
@@ -58,7 +59,7 @@ struct RunSmemLayout {
         off_popT = o; o += NP * D * 8;
         off_box = o; o += 3 * 8 * 8;               // flags[8], lo[8], hi[8]
         off_fit = o; o += NP * 8;                  // objective values of the members, fp64
-        off_part = o; o += (threads > NP ? threads : NP) * 8;      // [slice][candidate] partial sums, fp64
+        off_part = o; o += NP * slices * 8;        // [slice][candidate] partial sums, fp64
         off_xpart = o; o += (K > 1) ? 2 * K * NP * 8 : 0;           // [2][K][NP]: the cluster peers' sums, double-buffered
         total = align_up(o, 16);
     }
@@ -137,15 +138,16 @@ __device__ __forceinline__ float run_d2f(const double v) {
 
 // One evaluation pass over a tile of samples that sits in shared memory: xs[0 .. len_t) are samples n_t0 .. n_t0 + len_t of the
 // data block (the whole block, a cluster CTA's slice of it, or one tile of the streamed ring).  Work item = (candidate, slice):
-// with S = max(1, threads / NP) slices the tile is cut into S contiguous ranges on 4-sample boundaries; item i is candidate
-// i % NP over slice i / NP, and thread t takes items t, t + threads, ...  The item's sum goes to part[i] (added when `accumulate`).
+// the tile is cut into S = p.Ws contiguous ranges on 4-sample boundaries (the planner picks S so that NP x S items fill the
+// threads of the CTA in whole rounds); item i is candidate i % NP over slice i / NP, and thread t takes items t, t + threads, ...
+// The item's sum goes to part[i] (added when `accumulate`).
 // Not inlined: the loop's register allocation then does not depend on the code around it.
 template <int D, int AMP, bool CUB>
 __device__ PT_RUN_INLINE void run_eval_tile(const BlockParams& p, const float* __restrict__ xs, const int n_t0, const int len_t,
                                           const double* __restrict__ pop, double* __restrict__ part, const bool accumulate, const int tid,
                                           const int nthr) {
     const int NP = p.NP;
-    const int S = nthr > NP ? nthr / NP : 1;
+    const int S = p.Ws;
     const int quads = (len_t + 3) >> 2;
     const f32x2 neg1 = run_bc2(-1.0f);
     for (int item = tid; item < NP * S; item += nthr) {
@@ -260,7 +262,7 @@ __global__ void __launch_bounds__(kRunMaxThreads, 1) pt_run_kernel(const BlockPa
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int warp = tid >> 5, lane = tid & 31;
-    const RunSmemLayout L(p.NpadS, p.NP, D, nthr, p.TS, p.S, p.K);
+    const RunSmemLayout L(p.NpadS, p.NP, D, p.Ws, p.TS, p.S, p.K);
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem + L.off_bar);
     float* xs = reinterpret_cast<float*>(smem + L.off_xs);
     double* popA = reinterpret_cast<double*>(smem + L.off_popA);
@@ -284,7 +286,7 @@ __global__ void __launch_bounds__(kRunMaxThreads, 1) pt_run_kernel(const BlockPa
     const int n_hi = min(p.N, (int)(((long long)(rank + 1) * quads_blk) / K) * 4);
     const int Nown = n_hi - n_lo;
     uint32_t xchg = 0;             // exchanges of partial sums done so far (selects the xpart buffer)
-    const int S_sl = nthr > p.NP ? nthr / p.NP : 1;      // slices of the evaluation (run_eval_tile)
+    const int S_sl = p.Ws;         // slices of the evaluation (run_eval_tile)
 
     RunStream st;
     if (STREAM) {

@@ -94,6 +94,8 @@ def lib():
     L.pt_track_auto_host.restype = i32
     L.pt_fit_blocks_plan.argtypes = [i64, i32, C.POINTER(DEConfig), p]
     L.pt_fit_blocks_plan.restype = i32
+    L.pt_fit_blocks_launches.argtypes = [i64, i32, C.POINTER(DEConfig), p, i32]
+    L.pt_fit_blocks_launches.restype = i32
     L.pt_doppler_products.argtypes = [p, i64, i32, f64, f64, p, i32, p, p, p, p]
     L.pt_doppler_products.restype = i32
     L.pt_track_host.argtypes = [p, i64, i32, f64, p, p, C.POINTER(DEConfig), f64, p, i32, p, p, p, p, p, p]
@@ -272,6 +274,15 @@ def pt_fit_blocks_plan(B: int, N: int, cfg: DEConfig) -> dict:
     _check(lib().pt_fit_blocks_plan(B, N, C.byref(cfg), out), "pt_fit_blocks_plan")
     return dict(grid=out[0], threads=out[1], smem=out[2], resident=out[3], cands_per_thread=out[4], ctas_per_sm=out[5],
                 cluster=out[6], tail_cluster=out[7])
+
+
+def pt_fit_blocks_launches(B: int, N: int, cfg: DEConfig) -> list:
+    """The DE-kernel launches of pt_fit_blocks: [dict(first, blocks, grid, threads, cluster), ...] (include/pt.h)."""
+    out = (C.c_int32 * (5 * 16))()
+    n = lib().pt_fit_blocks_launches(B, N, C.byref(cfg), out, 16)
+    _check(min(n, 0), "pt_fit_blocks_launches")
+    return [dict(first=out[5 * k], blocks=out[5 * k + 1], grid=out[5 * k + 2], threads=out[5 * k + 3], cluster=out[5 * k + 4])
+            for k in range(min(n, 16))]
 
 
 def pt_doppler_products(best: torch.Tensor, T: float, los_scale: float = 0.0, blocks_per_interval=()):
