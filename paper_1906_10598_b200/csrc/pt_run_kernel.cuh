@@ -258,7 +258,7 @@ __device__ __forceinline__ void run_stream_issue_one(const BlockParams& p, RunSt
 }
 
 template <int D, int MODE, bool STREAM, int OBJ>
-__global__ void __launch_bounds__(kRunMaxThreads, 1) pt_run_kernel(const BlockParams p) {
+__global__ void __launch_bounds__(kRunMaxThreads, 1) pt_run_kernel(const __grid_constant__ BlockParams p) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int warp = tid >> 5, lane = tid & 31;
