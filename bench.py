@@ -37,7 +37,7 @@ SM_MAX_MHZ = 1965.0
 XU_PEAK = SM_COUNT * XU_LANES_PER_SM * SM_MAX_MHZ * 1e6     # 4.65e12 sample-evaluations/s, DESIGN.md "Roofline"
 # dram__bytes_read.sum + dram__bytes_write.sum of the DE-kernel launches of one step, from an `ncu --set full` capture of the
 # same command (profile file named beside the number); reported as roofline.traffic_ncu, never as a live measurement
-NCU_TRAFFIC = {"config2": {"bytes": 2.31e8, "source": "profiles/r2_bench_launches.md (the two DE-kernel launches of one step)"}}
+NCU_TRAFFIC = {"config2": {"bytes": 2.55e8, "source": "profiles/r2_bench_launches.md (the two DE-kernel launches of one step: 244.5 MB read + 10.5 MB written)"}}
 
 
 def kernel_name(plan: dict, wl) -> str:
