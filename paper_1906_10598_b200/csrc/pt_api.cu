@@ -97,9 +97,14 @@ static int device_info(int* sms, int* smem_optin, int* dev_out = nullptr) {
     return 0;
 }
 
+static bool have_device() {
+    int n = 0;
+    if (cudaGetDeviceCount(&n) != cudaSuccess || n == 0) { (void)cudaGetLastError(); return false; }
+    return true;
+}
 static int device_smem_optin() {
     int sms = 148, smem_optin = 232448;
-    if (device_info(&sms, &smem_optin)) return 232448;
+    if (!have_device() || device_info(&sms, &smem_optin)) return 232448;
     return smem_optin;
 }
 
@@ -527,9 +532,11 @@ static int run_launch_list(long long B, int N, int NP, int D, int sms, int smem_
         if (left * 2 <= sms) {
             // the last few blocks: clusters, as many CTAs per block as are resident at once
             bool ok = false;
-            for (int K = (int)(sms / left) < 8 ? (int)(sms / left) : 8; K >= 2 && !ok; --K) {
+            int Kmax = (int)(sms / left) < 8 ? (int)(sms / left) : 8;
+            if (Kmax > N / (2 * kRun)) Kmax = N / (2 * kRun);           // every CTA keeps at least two runs of samples
+            for (int K = Kmax; K >= 2 && !ok; --K) {
                 if (make_plan_run(left, N, NP, D, sms, smem_optin, K, &sg.pl) || sg.pl.K != K) continue;
-                ok = fit_max_resident_clusters(sg.pl, D) >= left;
+                ok = !have_device() || fit_max_resident_clusters(sg.pl, D) >= left;      // no device: the plan of a B200, residency assumed
             }
             if (!ok && make_plan_run(left, N, NP, D, sms, smem_optin, 1, &sg.pl, 1)) return 1;
             sg.count = left;
@@ -711,20 +718,21 @@ int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg, int32_
     Plan pl;
     rc = plan_for(B, N, cfg->NP, cfg->D, &pl, false, 0, cfg->objective);
     if (rc) return rc;
-    out[0] = pl.grid; out[1] = pl.threads; out[2] = pl.smem; out[3] = pl.resident; out[4] = pl.C; out[5] = pl.ctas_per_sm;
-    out[6] = pl.K; out[7] = 0;
-    int dev_count = 0;
-    if (cudaGetDeviceCount(&dev_count) == cudaSuccess && dev_count > 0) {
+    out[7] = 0;
+    if (pl.run) {
+        // the plan of the FIRST launch of the launch list (run_launch_list), and the cluster size of the last one
+        std::vector<Segment> segs;
+        if (force_cluster() == 0 && pl.K == 1 && pl.S == 0 && run_launch_list(B, N, cfg->NP, cfg->D, pl.sms, device_smem_optin(), &segs) == 0 &&
+            !segs.empty()) {
+            pl = segs.front().pl;
+            if (segs.size() > 1 && segs.back().pl.K > 1) out[7] = segs.back().pl.K;
+        }
+    } else if (have_device()) {
         Plan tl;
-        if (pl.run) {
-            std::vector<Segment> segs;
-            if (force_cluster() == 0 && pl.K == 1 && pl.S == 0 && run_launch_list(B, N, cfg->NP, cfg->D, pl.sms, device_smem_optin(), &segs) == 0 &&
-                segs.size() > 1 && segs.back().pl.K > 1)
-                out[7] = segs.back().pl.K;
-        } else if (plan_tail(B, N, cfg->NP, cfg->D, pl, &tl) > 0) out[7] = tl.K;
-    } else {
-        (void)cudaGetLastError();
+        if (plan_tail(B, N, cfg->NP, cfg->D, pl, &tl) > 0) out[7] = tl.K;
     }
+    out[0] = pl.grid; out[1] = pl.threads; out[2] = pl.smem; out[3] = pl.resident; out[4] = pl.C; out[5] = pl.ctas_per_sm;
+    out[6] = pl.K;
     return PT_OK;
 }
 
@@ -733,14 +741,14 @@ int32_t pt_fit_blocks_launches(int64_t B, int32_t N, const pt_de_config* cfg, in
     int rc = check_common(B, N, 1.0, cfg->NP, cfg->D);
     if (rc) return rc;
     Plan pl;
-    rc = plan_for(B, N, cfg->NP, cfg->D, &pl, true, 0, cfg->objective);
+    rc = plan_for(B, N, cfg->NP, cfg->D, &pl, false, 0, cfg->objective);
     if (rc) return rc;
     std::vector<Segment> segs;
     if (pl.run && force_cluster() == 0 && pl.K == 1 && pl.S == 0) {
         if (run_launch_list(B, N, cfg->NP, cfg->D, pl.sms, device_smem_optin(), &segs)) { set_error("no launch plan"); return PT_ERR_UNSUPPORTED; }
     } else {
         Plan tl;
-        const long long rem = plan_tail(B, N, cfg->NP, cfg->D, pl, &tl);
+        const long long rem = have_device() ? plan_tail(B, N, cfg->NP, cfg->D, pl, &tl) : 0;
         segs.push_back(Segment{0, B - rem, pl});
         if (rem > 0) segs.push_back(Segment{B - rem, rem, tl});
     }

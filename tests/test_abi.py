@@ -119,6 +119,48 @@ def test_plan_is_computable_without_gpu(lib_path):
     assert plan["smem"] <= 232448
 
 
+@pytest.mark.parametrize("B,N,NP,D", [(3600, 16000, 128, 5), (36000, 10000, 128, 6), (1024, 1024, 32, 5), (1024, 1024, 128, 5),
+                                      (1024, 4096, 512, 5), (1024, 16384, 128, 5), (1024, 65536, 256, 5), (148, 400000, 400, 6),
+                                      (60, 10000, 100, 5), (1, 1000, 60, 5), (149, 16000, 128, 5), (296, 16000, 128, 5),
+                                      (297, 16000, 128, 5), (443, 10000, 128, 6), (593, 4096, 64, 5), (7, 8, 4, 5)])
+def test_launch_list_covers_every_block_once_with_full_grids(lib_path, B, N, NP, D):
+    """Host logic of pt_fit_blocks (run_launch_list in csrc/pt_api.cu; no device needed: the plan of a B200).  The launches are
+    contiguous, cover blocks 0..B-1 exactly once, never over-subscribe the SMs, and every launch but the last has an exactly full
+    grid -- except blocks so short that a generation is bound by the DE step (NP N <= 65536), whose remainder stays one round."""
+    from paper_1906_10598_b200 import pt
+    cfg = pt.make_config(D=D, NP=NP, generations=10, t0=-0.5 * N / 1000.0)
+    plan = pt.pt_fit_blocks_plan(B, N, cfg)
+    launches = pt.pt_fit_blocks_launches(B, N, cfg)
+    assert 1 <= len(launches) <= 6
+    nxt = 0
+    for k, ln in enumerate(launches):
+        assert ln["first"] == nxt and ln["blocks"] >= 1
+        nxt += ln["blocks"]
+        assert ln["threads"] in (256, 512, 1024) and 1 <= ln["cluster"] <= 8
+        cps = 1024 // ln["threads"]
+        assert ln["grid"] <= 148 * cps and ln["grid"] % ln["cluster"] == 0
+        if ln["cluster"] > 1:
+            assert ln["grid"] == min(ln["blocks"], 148 // ln["cluster"]) * ln["cluster"] or ln["grid"] == ln["blocks"] * ln["cluster"]
+        elif plan["resident"] and k + 1 < len(launches):
+            assert ln["grid"] == 148 * cps and ln["blocks"] % ln["grid"] == 0           # whole rounds of an exactly full grid
+    assert nxt == B
+    assert launches[0]["threads"] == plan["threads"] and launches[0]["grid"] == plan["grid"]
+    if B >= 148 * 4 and NP * N > 65536 and plan["resident"]:
+        tail = sum(ln["blocks"] for ln in launches[1:])
+        assert tail < 148 * (1024 // launches[0]["threads"])                                  # the first launch takes all whole rounds
+
+
+def test_slices_fill_the_threads_in_whole_rounds(lib_path):
+    """choose_slices: NP x S work items over the CTA's threads.  Seen from outside through the shared-memory size of the plan
+    (part[S][NP] fp64): NP = 400 on 1024 threads takes S = 5 (2000 items, two rounds) on the streamed paper-shaped blocks."""
+    from paper_1906_10598_b200 import pt
+    cfg = pt.make_config(D=6, NP=400, generations=10, t0=-1.0)
+    plan = pt.pt_fit_blocks_plan(148, 400000, cfg)
+    assert plan["resident"] == 0 and plan["threads"] == 1024
+    fixed = 128 + 3 * 8192 * 4 + 2 * 400 * 6 * 8 + 3 * 8 * 8 + 400 * 8          # barriers, ring, populations, box, fit
+    assert plan["smem"] - fixed == 400 * 5 * 8
+
+
 def test_product_path_has_no_oracle_import():
     """The package must not import, read or run anything under oracle/ (the oracle is test infrastructure)."""
     pkg = os.path.join(ROOT, "paper_1906_10598_b200")
