@@ -73,7 +73,7 @@ __device__ __forceinline__ f32x2 run_bc2(float v) { return pack2(v, v); }
 // One run of one candidate, two consecutive samples at a time.  The run's polynomial phase(j) = E0 + j (E1 + j (E2 + j E3)) is
 // evaluated by Horner's rule at EVEN j with packed coefficient pairs: lane 0 holds the coefficients themselves (sample j), lane 1
 // the same polynomial shifted by one sample (sample j + 1), so that one FFMA2 chain yields the phases of samples (j, j + 1) and j
-// enters as a broadcast scalar -- in a full run a 32-bit immediate of the unrolled instruction stream (SASS: FFMA2 R, R, -64, R).
+// enters as a broadcast scalar -- in a full run a 32-bit immediate of the unrolled instruction stream (SASS: FFMA2 R, R, -128, R).
 //   chi^2 (Eq. 4): r = A' cos(y) + x with the negated amplitude A'(j) = Ac + j G, acc += r^2;   correlation (Eq. 5-6): acc += x cos(y).
 struct RunCoef { f32x2 E0, E1, E2, E3, Ac, G; };
 
@@ -398,18 +398,22 @@ __global__ void __launch_bounds__(kRunMaxThreads, 1) pt_run_kernel(const __grid_
                 flags[6] = bad ? 1.0 : 0.0;
             }
         } else {
-            if (tid == 1 || tid == 5) {   // a1 == 0 for every given member; the largest |fddot|
-                if (tid < D) {
-                    const float* pp = p.pop_in + blk * (long long)p.NP * D + tid;
-                    float mn = pp[0], mx = pp[0];
-                    for (int i = 1; i < p.NP; ++i) { const float v = pp[(size_t)i * D]; mn = fminf(mn, v); mx = fmaxf(mx, v); }
-                    if (tid == 1) flags[7] = (mn == 0.0f && mx == 0.0f) ? 1.0 : 0.0;
-                    else flags[5] = ((kTwoPi / 6.0) * (double)fmaxf(fabsf(mn), fabsf(mx)) * dt * dt * dt * (double)(kRun / 2) * (kRun / 2) * (kRun / 2) > 1.0e-7) ? 1.0 : 0.0;
+            // a1 == 0 for every given member (warp 0); the largest |fddot| (warp 1, D = 6): the lanes stride over the members
+            if (warp < 2 && (warp == 0 || D == 6)) {
+                const int col = warp == 0 ? 1 : 5;
+                const float* pp = p.pop_in + blk * (long long)p.NP * D + col;
+                float amax = 0.0f;
+                for (int i = lane; i < p.NP; i += 32) amax = fmaxf(amax, fabsf(__ldg(pp + (size_t)i * D)));
+#pragma unroll
+                for (int off = 16; off >= 1; off >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, off));
+                if (lane == 0) {
+                    if (warp == 0) flags[7] = (amax == 0.0f) ? 1.0 : 0.0;
+                    else flags[5] = ((kTwoPi / 6.0) * (double)amax * dt * dt * dt * (double)(kRun / 2) * (kRun / 2) * (kRun / 2) > 1.0e-7) ? 1.0 : 0.0;
                 }
             }
-            if (tid == 32) flags[6] = 0.0;
+            if (tid == 64 % nthr) flags[6] = 0.0;
         }
-        if (D == 5 && tid == 33) flags[5] = 0.0;
+        if (D == 5 && tid == 65 % nthr) flags[5] = 0.0;
         __syncthreads();
 
         const bool a1z = (OBJ == kObjChi2) && flags[7] != 0.0;

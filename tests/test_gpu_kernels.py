@@ -12,6 +12,7 @@ import numpy as np
 import pytest
 
 import oracle
+from _observed import observed
 from paper_1906_10598_b200 import workloads as W
 
 torch = pytest.importorskip("torch")
@@ -158,6 +159,7 @@ def test_run_kernel_d6_fit_config3_and_cubic(pt):
         g = _fit(pt, wl, NP=96, generations=600, seed=5)
     o = oracle.fit_blocks(wl.x, wl.fs, wl.lo, wl.hi, NP=96, generations=600, seed=5, block_index=wl.block_index)
     ok = np.abs(g["best_rss"] - o["best_rss"]) / o["best_rss"] < FIT_REL_TOL
+    observed("blocks on the same optimum (bar >= 2)", ok.sum())
     assert ok.sum() >= 2, (g["best_rss"], o["best_rss"])
     assert np.max(np.abs(_wrap(g["best"][ok, 2] - o["best"][ok, 2]))) < PHI0_TOL
     assert np.max(np.abs(g["best"][ok, 3] - o["best"][ok, 3])) < F_TOL
@@ -179,6 +181,7 @@ def test_first_generations_follow_the_oracle(pt, kernel):
         o = oracle.fit_blocks(wl.x, wl.fs, wl.lo, wl.hi, NP=NP, generations=4, seed=21, block_index=wl.block_index, want_pop=True)
         same = np.all(g["final_pop"] == o["final_pop"].astype(np.float32), axis=-1)
         print("\n[%s trajectory %s] identical members after 4 generations: %.4f" % (kernel, wl.name, same.mean()))
+        observed("identical members (bar > 0.98)", round(float(same.mean()), 4))
         assert same.mean() > 0.98
         assert np.max(np.abs(g["final_fit"] - o["final_fit"]) / o["final_fit"]) < FIT_REL_TOL
 
@@ -206,6 +209,7 @@ def test_kernels_agree_with_each_other(pt):
             res[kernel] = _fit(pt, wl, NP=128, generations=1000, seed=8)
     for a, b in (("run", "classic"), ("run", "tc")):
         ok = ((res[a]["status"] & 2) == 0) & ((res[b]["status"] & 2) == 0)
+        observed("blocks on the same optimum (bar >= 36)", ok.sum())
         assert ok.sum() >= 36
         dphi, df = np.abs(_wrap(res[a]["best"][ok, 2] - res[b]["best"][ok, 2])), np.abs(res[a]["best"][ok, 3] - res[b]["best"][ok, 3])
         print("\n[%s vs %s] |dphi0| median %.1e max %.1e rad, |df| median %.1e max %.1e Hz" % (a, b, np.median(dphi), dphi.max(), np.median(df), df.max()))
@@ -232,5 +236,6 @@ def test_run_kernel_results_do_not_depend_on_the_launch_geometry(pt):
         assert pt.pt_fit_blocks_plan(w2.B, w2.N, cfg)["threads"] == 1024
         b = _fit(pt, w2, NP=32, generations=3, seed=12, want_pop=True)
     same = np.all(a["final_pop"][sub] == b["final_pop"], axis=-1)
+    observed("identical members (bar > 0.995)", round(float(same.mean()), 4))
     assert same.mean() > 0.995, same.mean()
     assert np.max(np.abs(a["final_fit"][sub] - b["final_fit"]) / b["final_fit"]) < 1e-5

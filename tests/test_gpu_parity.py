@@ -11,6 +11,7 @@ import numpy as np
 import pytest
 
 import oracle
+from _observed import observed
 from paper_1906_10598_b200 import workloads as W
 
 torch = pytest.importorskip("torch")
@@ -207,12 +208,14 @@ def test_fit_streamed_trajectory_and_full_fit(pt, no_cluster):
     g = _gpu_fit(pt, wl, generations=3, seed=4, want_pop=True)
     o = _oracle_fit(wl, generations=3, seed=4, want_pop=True)
     same = np.all(g["final_pop"] == o["final_pop"].astype(np.float32), axis=-1)
+    observed("identical members (bar > 0.98)", round(float(same.mean()), 4))
     assert same.mean() > 0.98, same.mean()
     assert np.max(np.abs(g["final_fit"] - o["final_fit"]) / o["final_fit"]) < FIT_REL_TOL
     g = _gpu_fit(pt, wl, seed=4)
     o = _oracle_fit(wl, seed=4)
     # NP = 32 for 200 generations does not always collapse; compare where both sides agree on the optimum's RSS
     ok = np.abs(g["best_rss"] - o["best_rss"]) / o["best_rss"] < FIT_REL_TOL
+    observed("blocks on the same optimum (bar >= 3)", ok.sum())
     assert ok.sum() >= 3, (g["best_rss"], o["best_rss"])
     assert np.max(np.abs(_wrap(g["best"][ok, 2] - o["best"][ok, 2]))) < PHI0_TOL
     assert np.max(np.abs(g["best"][ok, 3] - o["best"][ok, 3])) < F_TOL
@@ -280,6 +283,7 @@ def test_fit_cluster_follows_the_oracle(pt, K):
         g = _gpu_fit(pt, wl, generations=3, seed=9, want_pop=True)
         o = _oracle_fit(wl, generations=3, seed=9, want_pop=True)
         same = np.all(g["final_pop"] == o["final_pop"].astype(np.float32), axis=-1)
+        observed("identical members (bar > 0.98)", round(float(same.mean()), 4))
         assert same.mean() > 0.98, same.mean()
         assert np.max(np.abs(g["final_fit"] - o["final_fit"]) / o["final_fit"]) < FIT_REL_TOL
         wl = W.config0(cases=range(5))
@@ -297,6 +301,7 @@ def test_fit_cluster_persistent_loop_and_single_cta_agree(pt):
     with _forced_cluster(1):
         b = _gpu_fit(pt, wl, seed=4)
     ok = ((a["status"] & 2) == 0) & ((b["status"] & 2) == 0)         # both populations collapsed
+    observed("blocks on the same optimum (bar >= 36)", ok.sum())
     assert ok.sum() >= 36, ok.sum()
     assert np.max(np.abs(a["best_rss"][ok] - b["best_rss"][ok]) / b["best_rss"][ok]) < 1e-5
     assert np.max(np.abs(_wrap(a["best"][ok, 2] - b["best"][ok, 2]))) < PHI0_TOL
@@ -323,6 +328,7 @@ def test_tail_wave_is_fitted_by_clusters_and_matches_the_single_launch(pt):
     with _forced_cluster(1):
         b = _gpu_fit(pt, wl, generations=2, seed=6, want_pop=True)
     same = np.all(a["final_pop"] == b["final_pop"], axis=-1)
+    observed("identical members (bar > 0.99)", round(float(same.mean()), 4))
     assert same.mean() > 0.99
     assert np.max(np.abs(a["final_fit"] - b["final_fit"]) / b["final_fit"]) < 1e-5
     k = 7          # the 5 tail blocks and the last 2 of the full wave, against the oracle
@@ -372,6 +378,7 @@ def test_first_generations_follow_the_oracle_trajectory(pt, D):
         g = _gpu_fit(pt, wl, generations=G, seed=21, want_pop=True, F=F, CR=CR, NP=60)
         o = _oracle_fit(wl, generations=G, seed=21, want_pop=True, F=F, CR=CR, NP=60)
         same = np.all(g["final_pop"] == o["final_pop"].astype(np.float32), axis=-1)
+        observed("identical members (bar > 0.98)", round(float(same.mean()), 4))
         assert same.mean() > 0.98, same.mean()
         assert np.all(g["final_pop"] >= wl.lo[:, None, :].astype(np.float32) - 1e-6)
         assert np.all(g["final_pop"] <= wl.hi[:, None, :].astype(np.float32) + 1e-6)
@@ -542,6 +549,7 @@ def test_block_index_selects_the_stream_and_persistent_loop_is_consistent(pt):
         assert np.array_equal(gk["best"][0], g["best"][k])
     o = oracle.fit_blocks(wl.x[:5], wl.fs, wl.lo[:5], wl.hi[:5], NP=16, generations=12, seed=77, want_pop=True)
     same = np.all(g["final_pop"][:5] == o["final_pop"].astype(np.float32), axis=-1)
+    observed("identical members (bar > 0.9)", round(float(same.mean()), 4))
     assert same.mean() > 0.9
 
 

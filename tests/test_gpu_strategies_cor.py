@@ -10,6 +10,7 @@ import numpy as np
 import pytest
 
 import oracle
+from _observed import observed
 from paper_1906_10598_b200 import workloads as W
 
 torch = pytest.importorskip("torch")
@@ -79,6 +80,7 @@ def test_first_generations_follow_the_oracle_trajectory(pt, strategy, D):
         # config 3 (T = 0.1 s) does not observe fdot, fddot, a1 (R13): trials that differ only there have RSS values
         # inside the fp32 error, so more selections flip, and a flipped member spreads through the difference vectors
         floor = 0.97 if (D == 5 or G == 1) else 0.8
+        observed("identical members (bar > floor)", round(float(same.mean()), 4))
         assert same.mean() > floor, (strategy, G, same.mean())
         assert np.max(np.abs(g["final_fit"] - o["final_fit"])[same] / o["final_fit"][same]) < REL_TOL
         assert np.all(g["final_pop"] >= wl.lo[:, None, :].astype(np.float32) - 1e-6)
@@ -92,6 +94,7 @@ def test_best_guided_strategies_on_clusters(pt, strategy):
     with _forced_cluster(4):
         g, o = _both(pt, wl, wl.lo, wl.hi, NP=64, G=3, F=0.6, CR=0.9, seed=7, strategy=strategy)
     same = np.all(g["final_pop"] == o["final_pop"].astype(np.float32), axis=-1)
+    observed("identical members (bar > 0.97)", round(float(same.mean()), 4))
     assert same.mean() > 0.97
 
 
@@ -128,6 +131,7 @@ def test_table4_settings_with_the_papers_strategy(pt):
     g, o = _both(pt, wl, wl.lo, wl.hi, NP=60, G=200, F=0.5, CR=0.85, seed=4, strategy=3)
     ref = oracle.fit_blocks(wl.x, wl.fs, wl.lo, wl.hi, NP=60, generations=500, F=0.5, CR=0.9, seed=4)
     ok = np.abs(g["best_rss"] - o["best_rss"]) <= 1e-5 * o["best_rss"]
+    observed("fraction on the same optimum (bar >= 0.5)", ok.mean())
     assert ok.mean() >= 0.5
     assert np.max(np.abs(_wrap(g["best"][ok, 2] - o["best"][ok, 2]))) < PHI0_TOL
     assert np.max(np.abs(g["best"][ok, 3] - o["best"][ok, 3])) < F_TOL
@@ -227,6 +231,7 @@ def test_cor_fit_config0(pt, strategy):
     # generation 0 and the first generations: identical populations
     g, o = _both(pt, wl, lo, hi, NP=60, G=3, F=0.5, CR=0.9, seed=2, strategy=strategy, objective=1)
     same = np.all(g["final_pop"] == o["final_pop"].astype(np.float32), axis=-1)
+    observed("identical members (bar > 0.97)", round(float(same.mean()), 4))
     assert same.mean() > 0.97
     g, o = _both(pt, wl, lo, hi, NP=60, G=400, F=0.5, CR=0.9, seed=2, strategy=strategy, objective=1)
     assert np.max(np.abs(_wrap(g["best"][:, 2] - o["best"][:, 2]))) < PHI0_TOL

@@ -8,6 +8,7 @@ import numpy as np
 import pytest
 
 import oracle
+from _observed import observed
 from paper_1906_10598_b200 import workloads as W
 
 torch = pytest.importorskip("torch")
@@ -144,6 +145,7 @@ def test_tc_full_fit_vs_oracle(pt, make, seed):
     dphi, df = _wrap(g["best"][:, 2] - o["best"][:, 2]), g["best"][:, 3] - o["best"][:, 3]
     print("\n[tc fit %s] same optimum %d/%d, max |dphi0| %.2e rad, max |df| %.2e Hz, max dRSS %.2e" %
           (wl.name, same.sum(), wl.B, np.abs(dphi[same]).max(), np.abs(df[same]).max(), drss[same].max()))
+    observed("identical members (bar >= 0.9)", round(float(same.mean()), 4))
     assert same.mean() >= 0.9
     assert np.abs(dphi[same]).max() < PHI0_TOL and np.abs(df[same]).max() < F_TOL
     for k in range(wl.B):           # every result is valid: its objective is the oracle's at its own parameters
@@ -160,6 +162,7 @@ def test_tc_strategies_agree_with_the_classic_kernel(pt, strategy):
     a = _fit(pt, wl, "tc", seed=7, strategy=strategy, generations=300)
     b = _fit(pt, wl, "classic", seed=7, strategy=strategy, generations=300)
     same = np.abs(a["best_rss"] - b["best_rss"]) / b["best_rss"] < FIT_REL_TOL
+    observed("identical members (bar >= 0.75)", round(float(same.mean()), 4))
     assert same.mean() >= 0.75
     assert np.abs(_wrap(a["best"][same, 2] - b["best"][same, 2])).max() < PHI0_TOL
     assert np.abs(a["best"][same, 3] - b["best"][same, 3]).max() < F_TOL
@@ -245,4 +248,5 @@ def test_tc_main_launch_with_classic_cluster_tail(pt):
     o = oracle.fit_blocks(wl.x[[0, 200, 305]], wl.fs, wl.lo[[0, 200, 305]], wl.hi[[0, 200, 305]], NP=16, generations=6, seed=9,
                           block_index=np.array([0, 200, 305], dtype=np.uint32), want_pop=True)
     same = np.all(g["final_pop"][[0, 200, 305]] == o["final_pop"].astype(np.float32), axis=-1)
+    observed("identical members (bar > 0.9)", round(float(same.mean()), 4))
     assert same.mean() > 0.9
