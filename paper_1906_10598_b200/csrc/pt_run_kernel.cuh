@@ -163,6 +163,26 @@ __device__ PT_RUN_INLINE void run_eval_tile(const BlockParams& p, const float* _
         // block-relative index of the run's first sample, in both precisions (exact: < 2^24; a conversion would run on the XU pipe)
         double nd = (double)(n_t0 + nb);
         float nf = (float)(n_t0 + nb);
+        // D = 5: the full runs of a slice follow each other at a fixed step, so their re-expansions are carried instead of recomputed.
+        // frac(P(t_c)) lives in 64-bit fixed point (turns x 2^64: the integer addition wraps exactly where the phase does, so there is
+        // no range reduction) and advances by its first and second differences; E1 advances in fp64 by its constant step; E2 is a
+        // constant of the candidate.  Per run: four integer additions, one DADD and one double -> float instead of a serial chain of
+        // a dozen fp64 operations and three conversions.  Quantisation 2^-64 turns per addition; E0 is read off with 2^-23 turns.
+        unsigned long long Pfix = 0, d1fix = 0, d2fix = 0;
+        double e1s = 0.0, de1s = 0.0;
+        float E2s = 0.0f;
+        if (D == 5 && ne - nb >= kRun) {
+            const double dt = p.dt, step = (double)kRun * dt;
+            const double tc = fma(nd + (double)(kRun / 2), dt, p.t0);               // centre of the slice's first run
+            auto fix = [](const double v) -> unsigned long long { return __double2ull_rn((v - floor(v)) * 18446744073709551616.0); };
+            const double slope = fma(f2, tc, f1);                                   // P'(t_c) [turns / s]
+            Pfix = fix(fma(tc, fma(tc, 0.5 * f2, f1), c0));
+            d1fix = fix(fma(step, slope, 0.5 * f2 * step * step));                  // P(t_c + step) - P(t_c)
+            d2fix = fix(f2 * step * step);
+            e1s = (kTwoPi * dt) * slope;
+            de1s = (kTwoPi * dt) * f2 * step;
+            E2s = run_d2f((kTwoPi * dt * dt) * (0.5 * f2));
+        }
         for (int n0 = nb; n0 < ne; n0 += kRun, nd += (double)kRun, nf += (float)kRun) {
             f32x2 acc = run_bc2(0.0f);
             // The polynomial is re-expanded at sample h of the run (its centre; a short last run of a slice: ITS centre, so that a
@@ -210,7 +230,29 @@ __device__ PT_RUN_INLINE void run_eval_tile(const BlockParams& p, const float* _
                 return c;
             };
             if (n0 + kRun <= ne) {
-                const RunCoef c = coefficients((float)(kRun / 2), (double)(kRun / 2));
+                RunCoef c;
+                if (D == 5) {
+                    // coefficients of a full run from the carried state (see below): no fp64 chain, no range reduction
+                    const int sfrac = (int)((uint32_t)(Pfix >> 32) + 256u);                         // frac(P) in [-1/2, 1/2) turns x 2^32, + half a step
+                    const float kf = __int_as_float(0x4B400000 + (sfrac >> 9)) - 12582912.0f;       // ... x 2^23, rounded, exact in fp32
+                    const float E0 = kf * (float)(kTwoPi / 8388608.0), E1 = run_d2f(e1s);
+                    Pfix += d1fix; d1fix += d2fix; e1s += de1s;
+                    c.E0 = pack2(E0, (E0 + E1) + E2s);
+                    c.E1 = pack2(E1, fmaf(2.0f, E2s, E1));
+                    c.E2 = run_bc2(E2s);
+                    c.E3 = run_bc2(0.0f);
+                    if (AMP == kRunAmpLinear) {
+                        const float dtf = p.dtf, g1 = na1 * dtf;
+                        const float Ac = fmaf(na1, fmaf(nf + (float)(kRun / 2), dtf, p.t0f), na0);
+                        c.Ac = pack2(Ac, Ac + g1);
+                        c.G = run_bc2(g1);
+                    } else {
+                        c.Ac = run_bc2(na0);
+                        c.G = run_bc2(0.0f);
+                    }
+                } else {
+                    c = coefficients((float)(kRun / 2), (double)(kRun / 2));
+                }
                 run_full<AMP, CUB>(xs + n0, c, acc);
             } else {
                 const int len = ne - n0, h = len >> 1;
