@@ -142,7 +142,7 @@ static bool want_run() {
     return o == 0 || o == 3;
 }
 
-// Plan of pt_run_kernel: one CTA of 1024 threads per SM, or 2 x 512 / 4 x 256 when shared memory and the number of blocks allow (the
+// Plan of pt_run_kernel: one CTA of 1024 threads per SM, or 2 x 512 / 4 x 256 / 8 x 128 (short blocks) when shared memory and the number of blocks allow (the
 // DE step of one CTA then overlaps with the evaluation of the others); with few blocks a cluster of K CTAs per block; blocks
 // larger than shared memory are streamed through a ring of 3 tiles.
 // Sample slices of pt_run_kernel's evaluation: NP x S work items over `threads` threads, `len` samples per tile.  Picks the S that
@@ -164,7 +164,13 @@ static int choose_slices(int NP, int threads, int len) {
     return best;
 }
 
-static int make_plan_run(long long B, int N, int NP, int D, int sms, int smem_optin, int force_K, Plan* pl, int max_cps = 4) {
+// Short blocks (measured on the config-4 sweep, profiles/r2_kernel_choice.md): with NP x N <= kRunCps8Max sample-evaluations per
+// generation a block runs on a CTA of 128 threads, eight per SM; with NP x N <= kRunPartialMax the remainder of a launch list stays
+// one partly filled round instead of being cut into exactly full grids of fewer, larger CTAs per SM (whose DE steps are exposed).
+constexpr long long kRunCps8Max = 1 << 18;
+constexpr long long kRunPartialMax = 1 << 19;
+constexpr int kRunMaxCps = 8;
+static int make_plan_run(long long B, int N, int NP, int D, int sms, int smem_optin, int force_K, Plan* pl, int max_cps = kRunMaxCps) {
     pl->sms = sms;
     pl->tc = 0; pl->tc_slots = 1; pl->run = 1;
     pl->C = 1; pl->NPpad = NP; pl->Wg = 1; pl->Ws = 1;
@@ -195,6 +201,9 @@ static int make_plan_run(long long B, int N, int NP, int D, int sms, int smem_op
         if (cps > 1 && B <= (long long)sms * (cps / 2)) continue;   // not enough blocks to want that many CTAs
         const int threads = kRunMaxThreads / cps;
         const int slices = choose_slices(NP, threads, N);
+        // eight CTAs of 128 threads: blocks so short that a generation is a few thousand cycles (slices of whole runs, and seven
+        // other CTAs evaluating while one is in its DE step)
+        if (cps == 8 && (long long)NP * N > kRunCps8Max) continue;
         const RunSmemLayout L(pl->Npad, NP, D, slices);
         if (L.total > smem_optin) continue;
         if ((long long)(L.total + 1024) * cps > per_sm_total) continue;
@@ -524,7 +533,7 @@ static long long plan_tail(long long B, int N, int NP, int D, const Plan& pl, Pl
 struct Segment { long long first, count; Plan pl; };
 static int run_launch_list(long long B, int N, int NP, int D, int sms, int smem_optin, std::vector<Segment>* out) {
     long long done = 0;
-    int max_cps = 4;
+    int max_cps = kRunMaxCps;
     while (done < B) {
         const long long left = B - done;
         Segment sg;
@@ -545,9 +554,10 @@ static int run_launch_list(long long B, int N, int NP, int D, int sms, int smem_
             const long long slots = (long long)sms * sg.pl.ctas_per_sm;
             if (left >= slots) {
                 sg.count = left / slots * slots;
-            } else if (sg.pl.ctas_per_sm > 1 && (long long)NP * N <= 65536) {
-                // blocks so short that a generation is bound by the latency of its DE step, not by the XU pipe (NP N / 14.4 cycles of
-                // evaluation against ~4500): larger CTAs would not run them faster, so the remainder stays one partly filled round
+            } else if (sg.pl.ctas_per_sm > 1 && (long long)NP * N <= kRunPartialMax) {
+                // blocks so short that a generation is bound by the latency of its DE step as much as by the XU pipe: fewer, larger
+                // CTAs per SM would expose it (measured: N 1024 NP 128, 4 + 2 + 1 CTAs per SM in three launches 68.8 %, one partly
+                // filled round of 8 per SM 76.6 %), so the remainder stays one partly filled round
                 sg.count = left;
             } else if (sg.pl.ctas_per_sm > 1) {
                 // fewer blocks than CTA slots: the largest c' <= left / SMs CTAs per SM, exactly full

@@ -19,7 +19,7 @@
 //     i.e. 6 FP32-pipe lane operations + 1 MUFU per sample-evaluation for D = 5 (pt_block_kernel: 7) and the same for D = 6 whenever
 //     the cubic term cannot matter inside a run (|E3| 128^3 below 1e-7 rad over the whole box: the run then carries the exact value,
 //     first and second derivative of the cubic at its centre); 7 otherwise.  4.75 issue slots per sample-evaluation (5.3);
-//   * 64 registers per thread: 32 warps per SM (one CTA of 1024 threads, or 2 x 512 / 4 x 256 for shorter blocks, whose DE steps
+//   * 64 registers per thread: 32 warps per SM (one CTA of 1024 threads, or 2 x 512 / 4 x 256 / 8 x 128 for shorter blocks, whose DE steps
 //     then overlap with the other CTAs' evaluation), against 16 warps of 128 registers in pt_block_kernel.
 // Every phase is rounded on its own: there is no recurrence.  (A forward-difference recurrence y += d, d += dd was measured first
 // and dropped: with dd below half an ulp of d the second difference is lost and the phase drifts by E2 j^2, 1e-5 rad at j = 64.

@@ -126,7 +126,8 @@ def test_plan_is_computable_without_gpu(lib_path):
 def test_launch_list_covers_every_block_once_with_full_grids(lib_path, B, N, NP, D):
     """Host logic of pt_fit_blocks (run_launch_list in csrc/pt_api.cu; no device needed: the plan of a B200).  The launches are
     contiguous, cover blocks 0..B-1 exactly once, never over-subscribe the SMs, and every launch but the last has an exactly full
-    grid -- except blocks so short that a generation is bound by the DE step (NP N <= 65536), whose remainder stays one round."""
+    grid -- except blocks so short that a generation is bound by the DE step (NP N <= 2^19), whose remainder stays one round;
+    blocks with NP N <= 2^18 run on CTAs of 128 threads, eight per SM."""
     from paper_1906_10598_b200 import pt
     cfg = pt.make_config(D=D, NP=NP, generations=10, t0=-0.5 * N / 1000.0)
     plan = pt.pt_fit_blocks_plan(B, N, cfg)
@@ -136,7 +137,7 @@ def test_launch_list_covers_every_block_once_with_full_grids(lib_path, B, N, NP,
     for k, ln in enumerate(launches):
         assert ln["first"] == nxt and ln["blocks"] >= 1
         nxt += ln["blocks"]
-        assert ln["threads"] in (256, 512, 1024) and 1 <= ln["cluster"] <= 8
+        assert ln["threads"] in (128, 256, 512, 1024) and 1 <= ln["cluster"] <= 8
         cps = 1024 // ln["threads"]
         assert ln["grid"] <= 148 * cps and ln["grid"] % ln["cluster"] == 0
         if ln["cluster"] > 1:
@@ -145,7 +146,9 @@ def test_launch_list_covers_every_block_once_with_full_grids(lib_path, B, N, NP,
             assert ln["grid"] == 148 * cps and ln["blocks"] % ln["grid"] == 0           # whole rounds of an exactly full grid
     assert nxt == B
     assert launches[0]["threads"] == plan["threads"] and launches[0]["grid"] == plan["grid"]
-    if B >= 148 * 4 and NP * N > 65536 and plan["resident"]:
+    if NP * N <= (1 << 18) and B > 148 * 4:
+        assert launches[0]["threads"] == 128
+    if B >= 148 * 4 and NP * N > (1 << 19) and plan["resident"]:
         tail = sum(ln["blocks"] for ln in launches[1:])
         assert tail < 148 * (1024 // launches[0]["threads"])                                  # the first launch takes all whole rounds
 

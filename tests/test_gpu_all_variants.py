@@ -64,8 +64,10 @@ CASES = {
     "run strategy 3 + correlation": (SMALL, dict(NP=16, G=3, strategy=3, objective=1, env={"PT_CLUSTER": "1"}), dict(cluster=1)),
     "run resident D6 (cubic folded into the run's second derivative)": (lambda: W.config3(blocks=[10, 11, 12]), dict(NP=16, G=2, D=6, env={"PT_CLUSTER": "1"}), dict(threads=1024)),
     "run more members than threads": (SMALL, dict(NP=1024, G=1, env={"PT_CLUSTER": "1"}), dict(threads=1024)),
+    "run 8 CTAs per SM (short blocks), one partly filled round": (lambda: W.single_tone_blocks(range(600), 2048, 2048.0, config=4, f_range=(20, 60)),
+                                                                  dict(NP=16, G=2), dict(threads=128, ctas_per_sm=8)),
     "run 4 CTAs per SM + cluster tail": (lambda: W.single_tone_blocks(range(600), 2048, 2048.0, config=4, f_range=(20, 60)),
-                                         dict(NP=16, G=2), dict(threads=256, ctas_per_sm=4, tail_cluster=lambda k: k >= 2)),
+                                         dict(NP=272, G=2), dict(threads=256, ctas_per_sm=4, tail_cluster=lambda k: k >= 2)),
     "run 2 CTAs per SM": (lambda: W.single_tone_blocks(range(160), 512, 512.0, config=4, f_range=(20, 60)), dict(NP=8, G=2), dict(threads=512, ctas_per_sm=2)),
     "run streamed ring": (lambda: W.single_tone_blocks(range(2), 65536, 65536.0, config=4), dict(NP=16, G=1, env={"PT_CLUSTER": "1"}), dict(resident=0, threads=1024)),
     "run streamed ring, quantised 4 bit": (lambda: W.single_tone_blocks(range(2), 65536, 65536.0, config=4), dict(NP=16, G=1, quant=4, env={"PT_CLUSTER": "1"}), dict(resident=0)),

@@ -220,17 +220,19 @@ def test_kernels_agree_with_each_other(pt):
 # ----------------------------------------------------------------------------------------------
 # launch geometries of pt_run_kernel
 # ----------------------------------------------------------------------------------------------
-def test_run_kernel_results_do_not_depend_on_the_launch_geometry(pt):
-    """700 short blocks on 4 CTAs per SM (+ the cluster tail) against the same blocks fitted 37 at a time (one 1024-thread CTA per
-    block): Philox streams depend on the block index only and the objective is summed in fp64 across slices, so the first
-    generations are the same populations."""
-    wl = W.config4(1024, 32, B=700, generations=3)
+@pytest.mark.parametrize("N,cps", [(1024, 8), (10240, 4)])
+def test_run_kernel_results_do_not_depend_on_the_launch_geometry(pt, N, cps):
+    """700 short blocks on 8 CTAs of 128 threads per SM (N = 1024: one partly filled round) or on 4 CTAs of 256 per SM (N = 10240: a
+    full grid + the remainder on larger CTAs) against the same blocks fitted 37 at a time (one 1024-thread CTA per block): Philox
+    streams depend on the block index only and the objective is summed in fp64 across slices, so the first generations are the same
+    populations."""
+    wl = W.config4(N, 32, B=700, generations=3)
     cfg = pt.make_config(D=5, NP=32, generations=3, seed=12, t0=wl.t0)
     plan = pt.pt_fit_blocks_plan(wl.B, wl.N, cfg)
-    assert plan["ctas_per_sm"] == 4 and plan["threads"] == 256, plan
+    assert plan["ctas_per_sm"] == cps and plan["threads"] == 1024 // cps, plan
     a = _fit(pt, wl, NP=32, generations=3, seed=12, want_pop=True)
     sub = list(range(0, 700, 19))
-    w2 = W.config4(1024, 32, B=700, generations=3)
+    w2 = W.config4(N, 32, B=700, generations=3)
     w2.x, w2.lo, w2.hi, w2.truth, w2.block_index = wl.x[sub], wl.lo[sub], wl.hi[sub], wl.truth[sub], wl.block_index[sub]
     with _env("run", "1"):
         assert pt.pt_fit_blocks_plan(w2.B, w2.N, cfg)["threads"] == 1024
@@ -238,4 +240,10 @@ def test_run_kernel_results_do_not_depend_on_the_launch_geometry(pt):
     same = np.all(a["final_pop"][sub] == b["final_pop"], axis=-1)
     observed("identical members (bar > 0.995)", round(float(same.mean()), 4))
     assert same.mean() > 0.995, same.mean()
-    assert np.max(np.abs(a["final_fit"][sub] - b["final_fit"]) / b["final_fit"]) < 1e-5
+    # The slices differ (8 x 128 threads: four full runs of 256 samples; 1024 threads: sixteen short runs of 64), and so do the
+    # expansion points of the fp32 phases: a full run sees phases up to pi + 128 |E1| = 160 rad at these 0.2 cycles per sample, half
+    # an ulp of which is 7.6e-6 rad, a 64-sample run a quarter of that.  Both geometries evaluate the same fp64 members, so they may
+    # differ by the larger error (DESIGN.md 5.13 measured <= 8.4e-6 against fp64 at this rate, either sign).
+    d_ab = np.max(np.abs(a["final_fit"][sub] - b["final_fit"]) / b["final_fit"])
+    observed("objective, geometry vs geometry (bar < 3e-5)", float(d_ab))
+    assert d_ab < 3e-5
