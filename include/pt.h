@@ -252,6 +252,27 @@ PT_API int32_t pt_refit_doubtful(const float* x, int64_t B, int32_t N, double fs
                           int32_t* attempts, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * pt_refit_doubtful_static -- pt_refit_doubtful for callers that cannot allocate device memory (code under CUDA graph capture,
+ * serving loops, harnesses that forbid cudaMalloc): same arguments without the workspace, same kernels in the same order on the
+ * same stream, identical results.  The scratch of the continuity check (Eq. 8 border residuals [B][10] fp64,
+ * running phase, doubtful flags, the ordered list of doubtful blocks and its length) lives in a file-scope device array of
+ * PT_STATIC_SCRATCH_BYTES (csrc/pt_noalloc.cu) that every GPU which loads the library holds until the process exits.
+ * The call itself allocates nothing (no cudaMalloc / cudaFree, no allocating library routine).
+ * Limit: pt_refit_doubtful_workspace_bytes(B, N, cfg) <= PT_STATIC_SCRATCH_BYTES, i.e. about 43 000 blocks that fit in shared
+ * memory (96 bytes per block; blocks streamed from global memory need rows of their own and are refused); beyond it the call
+ * returns PT_ERR_UNSUPPORTED with a message and launches nothing.
+ * All calls on a device share the array and it keeps the last call's contents: the bytes a call uses are cleared first, on the
+ * caller's stream.  Calls that overlap on the GPU (different streams with no dependency between them) race on it.
+ * pt_static_scratch_bytes() returns the compiled size.
+ */
+#define PT_STATIC_SCRATCH_BYTES (4 * 1024 * 1024)
+PT_API size_t pt_static_scratch_bytes(void);
+PT_API int32_t pt_refit_doubtful_static(const float* x, int64_t B, int32_t N, double fs, double* lo, double* hi,
+                                 const uint32_t* block_index, const pt_de_config* cfg /*[host]*/,
+                                 const pt_retry_config* retry /*[host]*/, double* best, float* best_rss, uint32_t* status,
+                                 int32_t* attempts, void* stream);
+
+/*
  * pt_doppler_products -- observables from the fitted parameters, fp64 throughout.  T = N/fs.
  *     phi(t) = phi0 + 2 pi (f t + fdot t^2/2 + fddot t^3/6),  F(t) = dphi/dt  [rad/s]    PAPER.md:228-234 (Eq. 7)
  *     border values at t = -T/2, +T/2, phases reduced to [0, 2 pi)                      PAPER.md:237-246 (Eq. 8)

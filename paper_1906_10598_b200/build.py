@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpt.so")
 STAMP = os.path.join(HERE, ".libpt.stamp")
-SOURCES = ["pt_api.cu", "pt_doppler.cu", "pt_acquire.cu", "pt_retry.cu"]
+SOURCES = ["pt_api.cu", "pt_doppler.cu", "pt_acquire.cu", "pt_retry.cu", "pt_noalloc.cu"]
 # bench-only micro-benchmarks (measured FFMA / MUFU stream rates): their own library, not part of the product ABI
 PROBE_LIB = os.path.join(HERE, "libpt_probe.so")
 PROBE_STAMP = os.path.join(HERE, ".libpt_probe.stamp")

@@ -89,6 +89,10 @@ def lib():
     L.pt_refit_doubtful_workspace_bytes.restype = sz
     L.pt_refit_doubtful.argtypes = [p, i64, i32, f64, p, p, p, C.POINTER(DEConfig), C.POINTER(RetryConfig), p, p, p, p, p, sz, p]
     L.pt_refit_doubtful.restype = i32
+    L.pt_static_scratch_bytes.argtypes = []
+    L.pt_static_scratch_bytes.restype = sz
+    L.pt_refit_doubtful_static.argtypes = [p, i64, i32, f64, p, p, p, C.POINTER(DEConfig), C.POINTER(RetryConfig), p, p, p, p, p]
+    L.pt_refit_doubtful_static.restype = i32
     L.pt_track_auto_host.argtypes = [p, i64, i32, f64, C.POINTER(DEConfig), C.POINTER(AcqConfig), C.POINTER(RetryConfig), f64, p,
                                      i32, p, p, p, p, p, p, p, p, p]
     L.pt_track_auto_host.restype = i32
@@ -266,6 +270,21 @@ def pt_refit_doubtful(x: torch.Tensor, fs: float, lo: torch.Tensor, hi: torch.Te
                                  _dev(fit["status"], torch.int32, "status"), attempts.data_ptr(), ws.data_ptr(), ws_bytes,
                                  _stream())
     _check(rc, "pt_refit_doubtful")
+    return attempts
+
+
+def pt_refit_doubtful_static(x: torch.Tensor, fs: float, lo: torch.Tensor, hi: torch.Tensor, cfg: DEConfig, retry: RetryConfig,
+                             fit: dict, attempts: torch.Tensor, *, block_index: torch.Tensor | None = None) -> torch.Tensor:
+    """pt_refit_doubtful without a workspace: the scratch is the library's static device array (include/pt.h), nothing is
+    allocated -- here neither: `attempts` [B] int32 is the caller's.  Returns `attempts`."""
+    B, N = x.shape
+    bidx = None if block_index is None else _dev(block_index, torch.int32, "block_index")
+    rc = lib().pt_refit_doubtful_static(_dev(x, torch.float32, "x"), B, N, float(fs), _dev(lo, torch.float64, "lo"),
+                                        _dev(hi, torch.float64, "hi"), bidx, C.byref(cfg), C.byref(retry),
+                                        _dev(fit["best"], torch.float64, "best"), _dev(fit["best_rss"], torch.float32, "best_rss"),
+                                        _dev(fit["status"], torch.int32, "status"), _dev(attempts, torch.int32, "attempts"),
+                                        _stream())
+    _check(rc, "pt_refit_doubtful_static")
     return attempts
 
 
