@@ -37,7 +37,7 @@ SM_MAX_MHZ = 1965.0
 XU_PEAK = SM_COUNT * XU_LANES_PER_SM * SM_MAX_MHZ * 1e6     # 4.65e12 sample-evaluations/s, DESIGN.md "Roofline"
 # dram__bytes_read.sum + dram__bytes_write.sum of the DE-kernel launches of one step, from an `ncu --set full` capture of the
 # same command (profile file named beside the number); reported as roofline.traffic_ncu, never as a live measurement
-NCU_TRAFFIC = {"config2": {"bytes": 2.55e8, "source": "profiles/r2_bench_launches.md (the two DE-kernel launches of one step: 244.5 MB read + 10.5 MB written)"}}
+NCU_TRAFFIC = {"config2": {"bytes": 2.497e8, "source": "profiles/r2_bench_launches.md (the two DE-kernel launches of one step: 243.5 MB read + 6.1 MB written)"}}
 
 
 def kernel_name(plan: dict, wl) -> str:
@@ -111,7 +111,7 @@ def make_workload(name: str, case: int):
         return wl
     if name == "config1_ncu":    # config 1 (60 blocks: clusters of 2 CTAs per block), 100 generations
         return W.config1(case=case, generations=100)
-    if name == "sweep1k_ncu":    # config-4 sweep point N = 1024, NP = 128 (4 CTAs per SM)
+    if name == "sweep1k_ncu":    # config-4 sweep point N = 1024, NP = 128 (8 CTAs of 128 threads per SM)
         return W.config4(1024, 128, B=1024, generations=200)
     if name == "config2_2w":     # two waves of config-2 blocks (the tensor-core kernel fits two blocks per CTA at a time)
         return W.config2(blocks=range(296), case=case, generations=100)
