@@ -355,7 +355,8 @@ PT_API int32_t pt_fit_blocks_plan(int64_t B, int32_t N, const pt_de_config* cfg 
 /* The DE-kernel launches pt_fit_blocks issues for B blocks (for reporting; without a device: the list for a B200, with the
  * tail clusters assumed resident).  Blocks all take the same time, so the
  * library cuts them into segments whose grids are exactly full: whole rounds of SMs x c CTAs, the remainder with fewer, larger CTAs
- * per SM, the last few blocks on clusters.  Launch k is described by out[5 k .. 5 k + 4] = first block, number of blocks, grid,
+ * per SM, the last few blocks on clusters.  (Short blocks, NP N <= 2^19 sample-evaluations per generation, keep their remainder as one
+ * partly filled round; with NP N <= 2^18 a block runs on a CTA of 128 threads, eight per SM.)  Launch k is described by out[5 k .. 5 k + 4] = first block, number of blocks, grid,
  * threads per CTA, CTAs per data block (cluster size).  Returns the number of launches (at most `max_launches` are written), or a
  * negative pt_status.
  * Evaluation kernels (row a5: Eq. 2-4): pt_run_kernel (thread = candidate, run-local Horner; the automatic choice),
